@@ -1,0 +1,358 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement: fp64 cell-updates/s per RK2 step at 256^3 (BASELINE.json).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3|4|2|0]
+
+A "step" is one pass of the whole hot path (ghost fill, stage 1, ghost fill, stage 2 with fused
+CFL reduction, device-side dt) over the whole grid.  `value` is timed with CUDA events on the
+library's stream with the state already resident in HBM (hydro_run_steps); `e2e` is the same step
+through the C-ABI with HOST buffers: every timed step copies the state host->device
+(hydro_set_state from pinned memory), runs hydro_cfl_dt + hydro_step, and copies it back
+(hydro_get_state) -- the transfer pattern of the paper's Algorithm 2.
+One JSON line on stdout (rank 0).  N > 1: independent replicas, one per GPU (DESIGN.md section 9:
+"replicas only"; the path has no exchange step on one domain), no data-path collective.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fp64 cell-updates/sec per RK2 step at 256^3; achieved HBM GB/s vs B200 peak"
+UNIT = "cell-updates/s"
+# algorithmic HBM bytes per cell: stage 1 reads U0 and writes U1 (2 x 40 B),
+# stage 2 reads U1 and U0 and writes U(n+1) (3 x 40 B)
+BYTES_STAGE = {1: 80.0, 2: 120.0}
+# fp64-pipe instructions per cell per stage of the ideal fused path
+FP64_LANES_PER_SM, N_SM = 64, 148
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md)", 1965.0
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "50"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.perf_counter(), line.strip()))
+
+    def stop(self, t0=None, t1=None):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.08)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        rows = [r for (t, r) in self.rows if (t0 is None or t >= t0) and (t1 is None or t <= t1)]
+        if not rows:
+            rows = [r for _, r in self.rows]
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)),
+                "power_w_max": float(max(pw)), "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def workload(idx):
+    from paper_1812_07977_b200 import inputs
+    cfg = inputs.config(idx)
+    return cfg
+
+
+def cfg_dict(cfg, extra=None):
+    d = {"workload": f"BASELINE.json configs[{cfg.index}]: {cfg.name}", "grid": list(cfg.shape),
+         "gamma": cfg.gamma, "cfl": cfg.cfl, "bc": list(cfg.bc), "limiter_theta": cfg.theta,
+         "l2": "state (2 padded buffers) larger than L2; no flush needed"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ------------------------------------------------------------------------------------------
+# oracle legs (the only places bench.py may execute oracle/)
+# ------------------------------------------------------------------------------------------
+
+def oracle_slab_state(cfg, nzs):
+    """Bounded sample of the workload: the central nzs z-planes of the config's initial state."""
+    U = cfg.state()
+    nz = cfg.shape[2]
+    z0 = (nz - nzs) // 2
+    return np.ascontiguousarray(U[:, z0:z0 + nzs])
+
+
+def time_oracle(cfg, steps, warmup, nzs):
+    import oracle
+    U = oracle_slab_state(cfg, nzs)
+    nx, ny = cfg.shape[0], cfg.shape[1]
+    o = oracle.OracleHydro(nx, ny, nzs, cfg.gamma, cfg.dx, cfg.bc)
+    o.set_cfl(cfg.cfl)
+    o.set_state(U)
+    for _ in range(warmup):
+        o.step(o.cfl_dt())
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        o.step(o.cfl_dt())
+    el = time.perf_counter() - t0
+    cells = nx * ny * nzs
+    return cells * steps / el, el, oracle.get_threads(), cells
+
+
+def cpu_baseline(cfg, budget_s=15.0):
+    """Oracle as it stands on the host cores, on a bounded sample (~10-30 s of CPU work)."""
+    nz = cfg.shape[2]
+    nzs = min(nz, 32)
+    rate, _, cores, _ = time_oracle(cfg, 1, 0, nzs)              # calibrate (also warms up)
+    plane = cfg.shape[0] * cfg.shape[1]
+    steps = 2
+    nzs = int(max(8, min(nz, budget_s * rate / (plane * steps))))
+    rate, el, cores, cells = time_oracle(cfg, steps, 0, nzs)
+    return {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"{cfg.name}: central {cfg.shape[0]}x{cfg.shape[1]}x{nzs} slab, {steps} RK2 "
+                      f"steps, {el:.1f} s wall"}
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    cfg = workload(args.config)
+    nz = cfg.shape[2]
+    rate, _, cores, _ = time_oracle(cfg, 1, 0, min(nz, 16))
+    plane = cfg.shape[0] * cfg.shape[1]
+    total = args.steps + args.warmup
+    nzs = int(max(8, min(nz, 120.0 * rate / (plane * total))))      # whole run ~2 min
+    rate, el, cores, cells = time_oracle(cfg, args.steps, args.warmup, nzs)
+    sample = (f"{cfg.name}: central {cfg.shape[0]}x{cfg.shape[1]}x{nzs} slab per step, "
+              f"{args.steps} timed RK2 steps")
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * el / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": cfg_dict(cfg, {"sample_cells_per_step": cells}),
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------
+# our arm
+# ------------------------------------------------------------------------------------------
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1812_07977_b200.binding import Hydro, load_library
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = workload(args.config)
+    L = load_library(False)
+    hbm_peak, peak_src, sm_max = load_peaks()
+    cells = cfg.cells
+
+    h = Hydro(*cfg.shape, cfg.gamma, cfg.dx, cfg.bc)
+    h.set_cfl(cfg.cfl)
+    if args.variant is not None:
+        h.set_kernel_variant(args.variant)
+    U0 = torch.from_numpy(cfg.state()).pin_memory()        # pinned host copy of the input
+    Ud = U0.cuda(non_blocking=True)
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps, state in HBM, device-side dt -----------------------
+    h.set_state(Ud)
+    h.run_steps(args.warmup)
+    h.set_state(Ud)                                        # same physical state every run
+    h.run_steps(max(args.warmup, 3))
+    L.hydro_set_profiling(h._h, 1)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.15)
+    n0 = h.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    tw0 = time.perf_counter()
+    ev0.record()
+    h.run_steps(args.steps)
+    ev1.record()
+    torch.cuda.synchronize()
+    tw1 = time.perf_counter()
+    barrier()
+    launches = h.launch_count() - n0
+    clocks = sampler.stop(tw0, tw1) if rank == 0 else None
+    ms = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * cells * args.steps / (ms * 1e-3)
+
+    # per-kernel durations recorded by the library with CUDA events on its own stream
+    import ctypes as C
+    kt = {}
+    for which, name in ((0, "ghost_fill"), (1, "stage1"), (2, "stage2"), (3, "next_dt")):
+        tms, cnt = C.c_double(), C.c_longlong()
+        L.hydro_get_kernel_time(h._h, which, C.byref(tms), C.byref(cnt))
+        kt[name] = (tms.value, cnt.value)
+    L.hydro_set_profiling(h._h, 0)
+    _, nsteps = h.get_time()
+    st_ms = kt["stage1"][0] + kt["stage2"][0]
+    st_n = kt["stage1"][1] + kt["stage2"][1]
+    roofline = None
+    if st_n:
+        bytes_pair = (BYTES_STAGE[1] + BYTES_STAGE[2]) * cells     # one stage-1 + one stage-2 launch
+        avg_pair_ms = st_ms / (st_n / 2)
+        achieved = bytes_pair / (avg_pair_ms * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                    "frac": achieved / hbm_peak, "traffic": args.traffic,
+                    "kernel": "stage_fused<1> + stage_fused<2> (one RK2 step's two stage launches)"
+                              if (args.variant is None or args.variant == 1) else "stage_simple<1,2>",
+                    "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
+                                                     "stage2": BYTES_STAGE[2] * cells},
+                    "avg_launch_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in kt.items()},
+                    "share_of_step": {k: v[0] / ms for k, v in kt.items()}}
+
+    # ---- end to end through the C-ABI with HOST buffers --------------------------------------
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    Uh = U0.clone().pin_memory()
+    out_h = torch.empty_like(Uh).pin_memory()
+    h.set_state(Uh); h.step(h.cfl_dt()); h.get_state(out_h)             # warm the copy path
+    barrier()
+    te0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        h.set_state(Uh)                                    # H2D of the step's input state
+        h.step(h.cfl_dt())                                 # + 8-byte D2H of max signal speed
+        h.get_state(out_h)                                 # D2H of the step's result
+        Uh, out_h = out_h, Uh
+    torch.cuda.synchronize()
+    te = time.perf_counter() - te0
+    t = torch.tensor([te], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    te = float(t.item())
+    state_bytes = 5 * cells * 8
+    e2e = {"value": world * cells * e2e_steps / te, "unit": UNIT,
+           "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes + 48,
+           "steps": e2e_steps, "ms_per_step": 1e3 * te / e2e_steps,
+           "what": "per step: hydro_set_state(pinned host) + hydro_cfl_dt + hydro_step + "
+                   "hydro_get_state(pinned host)"}
+
+    # whole-job variant: state uploaded once, K steps with host-side dt, state downloaded once
+    h.set_state(U0)
+    barrier()
+    tj0 = time.perf_counter()
+    h.set_state(U0)
+    for _ in range(args.steps):
+        h.step(h.cfl_dt())
+    h.get_state(out_h)
+    tj = time.perf_counter() - tj0
+    e2e["job"] = {"value": world * cells * args.steps / tj, "unit": UNIT, "steps": args.steps,
+                  "what": "hydro_set_state(host) once + K x (hydro_cfl_dt + hydro_step) + "
+                          "hydro_get_state(host) once"}
+
+    if rank == 0:
+        cpu = None
+        if world == 1 and not args.no_cpu_baseline:
+            cpu = cpu_baseline(cfg)
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps,
+                "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic",
+                "config": cfg_dict(cfg, {"parallelism": "single GPU" if world == 1 else
+                                         f"{world} independent replicas (no collective)",
+                                         "dt": "device-resident (hydro_run_steps)"}),
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+                "roofline": roofline, "cpu_baseline": cpu}
+        if roofline:
+            # fp64-pipe view of the same launches: instructions issued per
+            # cell-stage by the kernel as compiled x cells / time vs lanes x clock
+            clk = (clocks or {}).get("sm_mhz") or sm_max
+            line["hbm_gbs_whole_step"] = (BYTES_STAGE[1] + BYTES_STAGE[2]) * cells * args.steps / (ms * 1e-3) / 1e9
+            line["fp64_pipe_peak_ginstr_s"] = N_SM * FP64_LANES_PER_SM * clk * 1e6 / 1e9
+        print(json.dumps(line), flush=True)
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--variant", type=int, default=None)
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per stage-pair launch from the committed ncu --set full capture")
+    args = ap.parse_args()
+    if args.traffic is None:
+        p = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(p):
+            args.traffic = json.load(open(p)).get(f"config{args.config}")
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

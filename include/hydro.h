@@ -1,0 +1,135 @@
+/*
+ * hydro.h -- C-ABI boundary of the B200-native RK2 step of the 3D compressible-Euler
+ * finite-volume update (the hot path of the GenASiS RiemannProblem example,
+ * arXiv 1812.07977).
+ *
+ * The calls follow the paper's statement of the problem: Algorithm 1 "Fluid Evolution"
+ * -- Initialize / ComputeTimeStep / two Runge-Kutta substeps of
+ * {ComputeDifferences, ComputeReconstruction, ComputeFluxes, ComputeUpdate} separated by
+ * GhostExchange -- over persistently device-allocated storage with explicit, rare transfers
+ * (PAPER.md:23, 130, 247).  The numerics the paper does not print (limiter, Riemann solver,
+ * EOS, time-step formula) are BASELINE.json:north_star's, under the readings R1-R20 listed in
+ * DESIGN.md section 3.
+ *
+ * Conventions
+ *  - Every call returns an int status (HYDRO_OK = 0); results come back through out-pointers.
+ *  - Packed state layout for set/get: double U[5][nz][ny][nx], x fastest, ACTIVE cells only,
+ *    variable order (rho, m_x, m_y, m_z, E) ("Value(nCells,nVariables)").
+ *  - A `U` pointer may be a HOST pointer (pageable or pinned) or a DEVICE pointer on the
+ *    handle's device; the library detects which (cudaPointerGetAttributes).  The caller owns
+ *    `U` and may free or reuse it as soon as the call returns.
+ *  - The handle owns all device memory it allocates (two ghost-padded SoA buffers + scalars).
+ *  - Work is enqueued on the handle's stream (default: the legacy default stream; see
+ *    hydro_set_stream).  hydro_step / hydro_run_steps only enqueue; hydro_cfl_dt,
+ *    hydro_max_signal_speed, hydro_evolve, hydro_get_state and hydro_get_time synchronise
+ *    that stream.
+ *  - A handle is not thread-safe; distinct handles are independent.
+ *  - Deterministic: same inputs => bit-identical outputs run to run (the only atomic is an
+ *    integer max on the bit pattern of a non-negative double).
+ *  - There is no CPU fallback: without a CUDA device every call that needs one returns
+ *    HYDRO_ERR_CUDA.
+ */
+#ifndef HYDRO_B200_H
+#define HYDRO_B200_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hydro hydro_t;   /* opaque */
+
+/* Boundary rule per face (R9; replaces the physical-boundary part of the paper's
+ * GhostExchange). */
+enum { HYDRO_BC_OUTFLOW = 0, HYDRO_BC_REFLECT = 1, HYDRO_BC_PERIODIC = 2 };
+
+enum {
+    HYDRO_OK = 0,
+    HYDRO_ERR_ARG = 1,        /* bad argument (see each call) */
+    HYDRO_ERR_ALLOC = 2,      /* device or host allocation failed */
+    HYDRO_ERR_CUDA = 3,       /* a CUDA call failed; text in hydro_last_error() */
+    HYDRO_ERR_UNPHYSICAL = 4, /* rho <= 0, p <= 0 or a non-finite signal speed was seen */
+    HYDRO_ERR_NOSTATE = 5     /* step/evolve/cfl_dt/get_state before set_state */
+};
+
+/* ---- the calls BASELINE.json:north_star names -------------------------------------- */
+
+/* Algorithm 1 line 1, "Initialize": allocate the persistent device state for an
+ * nx*ny*nz grid of cubic cells of edge dx (R13) with 2 ghost layers per side,
+ * ideal gas with adiabatic index gamma (R1).
+ *   bc[6]: HYDRO_BC_* for faces xlo,xhi,ylo,yhi,zlo,zhi (host pointer, copied).
+ * Defaults: CFL 0.7, limiter theta 1.4.
+ * HYDRO_ERR_ARG if nx,ny,nz < 2, gamma <= 1, dx <= 0 or non-finite, unknown bc value,
+ * periodic on only one face of an axis, or a NULL pointer.  *out is NULL on failure. */
+int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6],
+                 hydro_t **out);
+
+/* Copy a packed state (host or device pointer, layout above) into the device state; resets the
+ * time to 0 and the step count to 0.  Synchronous for pageable host memory. */
+int hydro_set_state(hydro_t *h, const double *U);
+
+/* Algorithm 1 line 5, "ComputeTimeStep": reduction over active cells,
+ *   *dt = (cfl/3) * (dx / max(|v| + c_s))      (R8; |v| Euclidean, c_s = sqrt(gamma p/rho)).
+ * dt: host pointer.  Synchronises.  HYDRO_ERR_UNPHYSICAL if any active cell has rho <= 0,
+ * p <= 0 or a non-finite speed. */
+int hydro_cfl_dt(hydro_t *h, double *dt);
+
+/* One RK2 step of size dt: Algorithm 1 lines 6-21:
+ *   U1 = U0 + dU(U0);  U(n+1) = 0.5*(U0 + U1 + dU(U1)),  ghost fill before each substep.
+ * Asynchronous (enqueue only).  HYDRO_ERR_ARG if dt <= 0 or non-finite. */
+int hydro_step(hydro_t *h, double dt);
+
+/* Algorithm 1 lines 3-4, 23: while t < t_final { dt = cfl_dt; clip the
+ * last step to land on t_final exactly (R14); step }.  *nsteps (host, may be NULL) receives the
+ * number of steps taken.  Synchronises.  HYDRO_ERR_ARG if t_final < t or non-finite. */
+int hydro_evolve(hydro_t *h, double t_final, long long *nsteps);
+
+/* Copy the device state out into a packed array (host or device pointer).  Synchronises.
+ * Returns HYDRO_ERR_UNPHYSICAL (after copying) if the sticky unphysical flag is set. */
+int hydro_get_state(hydro_t *h, double *U);
+
+/* ---- needed but not named in north_star -------------------------------------------- */
+
+int hydro_destroy(hydro_t *h);
+int hydro_set_cfl(hydro_t *h, double cfl);               /* > 0; configs use 0.7 / 0.5 */
+int hydro_set_limiter_theta(hydro_t *h, double theta);   /* in [1,2]; default 1.4 (R5) */
+int hydro_get_time(hydro_t *h, double *t, long long *step);   /* either may be NULL */
+/* Raw reduction max(|v| + c_s) over active cells (test hook; same error rule as cfl_dt). */
+int hydro_max_signal_speed(hydro_t *h, double *smax);
+/* Run on this cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream).  NULL = default. */
+int hydro_set_stream(hydro_t *h, void *cuda_stream);
+/* Process-wide allocator hook used by handles created afterwards (e.g. torch's caching
+ * allocator).  alloc(bytes, stream) returns a device pointer or NULL; release(ptr) frees it.
+ * Pass NULL, NULL to restore cudaMalloc / cudaFree. */
+int hydro_set_allocator(void *(*alloc)(size_t bytes, void *stream), void (*release)(void *ptr));
+/* n steps with the time step kept on the device: each step uses
+ * dt = (cfl/3)*dx/smax with smax reduced by the previous step's last kernel (or by a
+ * stand-alone reduction after set_state).  No host round trip; asynchronous.  The benchmark
+ * path (Algorithm 1's loop body without the host-side ComputeTimeStep of Algorithm 2,
+ * PAPER.md:198). */
+int hydro_run_steps(hydro_t *h, long long n);
+/* Test hooks: run only the ghost fill on the current state, and read the padded buffer
+ * [5][nz+4][ny+4][nx+4] (x fastest, row pitch removed) into a host or device array. */
+int hydro_ghost_fill(hydro_t *h);
+int hydro_get_padded(hydro_t *h, double *Upad);
+/* Select the stage-kernel implementation: 0 = reference-structured simple kernel
+ * (one thread per cell, everything recomputed), 1 = fused tiled kernel (default). */
+int hydro_set_kernel_variant(hydro_t *h, int variant);
+/* Measurement hooks (bench.py): when enabled, every kernel launch of this handle is bracketed by
+ * CUDA events on the handle's stream.  hydro_get_kernel_time synchronises and returns the summed
+ * duration (ms) and launch count since profiling was enabled, for which = 0 ghost fill,
+ * 1 stage-1 kernel, 2 stage-2 kernel, 3 next-dt kernel, 4 stand-alone CFL reduction. */
+int hydro_set_profiling(hydro_t *h, int enable);
+int hydro_get_kernel_time(hydro_t *h, int which, double *ms, long long *count);
+/* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
+long long hydro_launch_count(void);
+/* 1 if this library was compiled with -fmad=false (verification build), else 0. */
+int hydro_is_verification_build(void);
+/* Text of the last error on this thread (never NULL). */
+const char *hydro_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HYDRO_B200_H */

@@ -1,0 +1,214 @@
+"""Thin ctypes binding over the C-ABI of include/hydro.h (argument marshalling only).
+
+Every step of the path runs in the CUDA library; nothing here computes.  PyTorch supplies device
+memory (its caching allocator is installed as the library's allocator hook) and the stream.
+There is no CPU fallback: if the library is not built, or no CUDA device is present, this raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+BC_OUTFLOW, BC_REFLECT, BC_PERIODIC = 0, 1, 2
+_ERR = {1: "HYDRO_ERR_ARG", 2: "HYDRO_ERR_ALLOC", 3: "HYDRO_ERR_CUDA", 4: "HYDRO_ERR_UNPHYSICAL",
+        5: "HYDRO_ERR_NOSTATE"}
+
+# every symbol include/hydro.h declares (tests check the library exports all of them)
+SYMBOLS = ["hydro_create", "hydro_set_state", "hydro_cfl_dt", "hydro_step", "hydro_evolve",
+           "hydro_get_state", "hydro_destroy", "hydro_set_cfl", "hydro_set_limiter_theta",
+           "hydro_get_time", "hydro_max_signal_speed", "hydro_set_stream", "hydro_set_allocator",
+           "hydro_run_steps", "hydro_ghost_fill", "hydro_get_padded", "hydro_set_kernel_variant",
+           "hydro_set_profiling", "hydro_get_kernel_time", "hydro_launch_count", "hydro_is_verification_build", "hydro_last_error"]
+
+
+class HydroError(RuntimeError):
+    def __init__(self, code, where, text=""):
+        super().__init__(f"{where}: {_ERR.get(code, code)} {text}".strip())
+        self.code = code
+
+
+_libs = {}
+_dp = C.POINTER(C.c_double)
+_ALLOC_T = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+_FREE_T = C.CFUNCTYPE(None, C.c_void_p)
+_hooks = {}
+
+
+def build(force=False):
+    return _build.build(force=force)
+
+
+def load_library(verify=False):
+    """dlopen the production (or -fmad=false verification) library; raises if it is not built."""
+    key = bool(verify)
+    if key in _libs:
+        return _libs[key]
+    path = _build.LIB_VERIFY if verify else _build.LIB
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is not built: run `python -m paper_1812_07977_b200.build` "
+                           "(there is no CPU fallback)")
+    L = C.CDLL(path)
+    vp = C.c_void_p
+    L.hydro_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
+                               C.POINTER(C.c_int), C.POINTER(vp)]
+    L.hydro_set_state.argtypes = [vp, vp]
+    L.hydro_get_state.argtypes = [vp, vp]
+    L.hydro_get_padded.argtypes = [vp, vp]
+    L.hydro_cfl_dt.argtypes = [vp, _dp]
+    L.hydro_max_signal_speed.argtypes = [vp, _dp]
+    L.hydro_step.argtypes = [vp, C.c_double]
+    L.hydro_evolve.argtypes = [vp, C.c_double, C.POINTER(C.c_longlong)]
+    L.hydro_destroy.argtypes = [vp]
+    L.hydro_set_cfl.argtypes = [vp, C.c_double]
+    L.hydro_set_limiter_theta.argtypes = [vp, C.c_double]
+    L.hydro_get_time.argtypes = [vp, _dp, C.POINTER(C.c_longlong)]
+    L.hydro_set_stream.argtypes = [vp, vp]
+    L.hydro_set_allocator.argtypes = [vp, vp]
+    L.hydro_run_steps.argtypes = [vp, C.c_longlong]
+    L.hydro_ghost_fill.argtypes = [vp]
+    L.hydro_set_kernel_variant.argtypes = [vp, C.c_int]
+    L.hydro_set_profiling.argtypes = [vp, C.c_int]
+    L.hydro_get_kernel_time.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_longlong)]
+    L.hydro_launch_count.restype = C.c_longlong
+    L.hydro_is_verification_build.restype = C.c_int
+    L.hydro_last_error.restype = C.c_char_p
+    _libs[key] = L
+    return L
+
+
+def use_torch_allocator(L):
+    """Install torch's caching allocator as the library's device-memory hook."""
+    import torch
+    key = id(L)
+    if key in _hooks:
+        return
+
+    def _alloc(nbytes, stream):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+        except Exception:
+            return None
+
+    def _free(ptr):
+        torch.cuda.caching_allocator_delete(int(ptr))
+
+    a, f = _ALLOC_T(_alloc), _FREE_T(_free)
+    _hooks[key] = (a, f)                      # keep the callbacks alive
+    rc = L.hydro_set_allocator(C.cast(a, C.c_void_p), C.cast(f, C.c_void_p))
+    if rc:
+        raise HydroError(rc, "hydro_set_allocator", L.hydro_last_error().decode())
+
+
+def _as_ptr(U, shape, writable=False):
+    """(pointer, keepalive, is_device) for a numpy array or a torch tensor of `shape`, fp64."""
+    if isinstance(U, np.ndarray):
+        if U.dtype != np.float64 or not U.flags.c_contiguous or (writable and not U.flags.writeable):
+            raise ValueError("need a C-contiguous float64 array")
+        if tuple(U.shape) != tuple(shape):
+            raise ValueError(f"shape {U.shape} != {shape}")
+        return C.c_void_p(U.ctypes.data), U, False
+    import torch
+    if isinstance(U, torch.Tensor):
+        if U.dtype != torch.float64 or not U.is_contiguous() or tuple(U.shape) != tuple(shape):
+            raise ValueError(f"need a contiguous float64 tensor of shape {shape}")
+        return C.c_void_p(U.data_ptr()), U, U.is_cuda
+    raise TypeError(type(U))
+
+
+class Hydro:
+    """hydro_t with the C-ABI's call names.  `verify=True` loads the -fmad=false build."""
+
+    def __init__(self, nx, ny, nz, gamma, dx, bc, verify=False, torch_allocator=True,
+                 stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: this library has no CPU fallback")
+        self._L = load_library(verify)
+        if torch_allocator:
+            torch.cuda.init()
+            use_torch_allocator(self._L)
+        self.shape = (5, nz, ny, nx)
+        self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
+        self._h = C.c_void_p()
+        arr = (C.c_int * 6)(*[int(b) for b in bc])
+        self._chk(self._L.hydro_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "hydro_create")
+        if stream is None:
+            stream = torch.cuda.current_stream().cuda_stream
+        self._chk(self._L.hydro_set_stream(self._h, C.c_void_p(stream)), "hydro_set_stream")
+
+    def _chk(self, rc, where):
+        if rc:
+            raise HydroError(rc, where, self._L.hydro_last_error().decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.hydro_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_cfl(self, cfl):
+        self._chk(self._L.hydro_set_cfl(self._h, cfl), "hydro_set_cfl")
+
+    def set_limiter_theta(self, theta):
+        self._chk(self._L.hydro_set_limiter_theta(self._h, theta), "hydro_set_limiter_theta")
+
+    def set_kernel_variant(self, variant):
+        self._chk(self._L.hydro_set_kernel_variant(self._h, variant), "hydro_set_kernel_variant")
+
+    def set_stream(self, cuda_stream):
+        self._chk(self._L.hydro_set_stream(self._h, C.c_void_p(cuda_stream)), "hydro_set_stream")
+
+    def set_state(self, U):
+        p, keep, _ = _as_ptr(U, self.shape)
+        self._chk(self._L.hydro_set_state(self._h, p), "hydro_set_state")
+
+    def get_state(self, out=None):
+        if out is None:
+            out = np.empty(self.shape)
+        p, keep, _ = _as_ptr(out, self.shape, writable=True)
+        self._chk(self._L.hydro_get_state(self._h, p), "hydro_get_state")
+        return out
+
+    def get_padded(self):
+        out = np.empty(self.padded_shape)
+        self._chk(self._L.hydro_get_padded(self._h, C.c_void_p(out.ctypes.data)), "hydro_get_padded")
+        return out
+
+    def ghost_fill(self):
+        self._chk(self._L.hydro_ghost_fill(self._h), "hydro_ghost_fill")
+
+    def cfl_dt(self):
+        dt = C.c_double()
+        self._chk(self._L.hydro_cfl_dt(self._h, C.byref(dt)), "hydro_cfl_dt")
+        return dt.value
+
+    def max_signal_speed(self):
+        s = C.c_double()
+        self._chk(self._L.hydro_max_signal_speed(self._h, C.byref(s)), "hydro_max_signal_speed")
+        return s.value
+
+    def step(self, dt):
+        self._chk(self._L.hydro_step(self._h, dt), "hydro_step")
+
+    def run_steps(self, n):
+        self._chk(self._L.hydro_run_steps(self._h, int(n)), "hydro_run_steps")
+
+    def evolve(self, t_final):
+        n = C.c_longlong()
+        self._chk(self._L.hydro_evolve(self._h, t_final, C.byref(n)), "hydro_evolve")
+        return n.value
+
+    def get_time(self):
+        t, n = C.c_double(), C.c_longlong()
+        self._chk(self._L.hydro_get_time(self._h, C.byref(t), C.byref(n)), "hydro_get_time")
+        return t.value, n.value
+
+    def launch_count(self):
+        return self._L.hydro_launch_count()

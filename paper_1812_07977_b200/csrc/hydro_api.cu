@@ -1,0 +1,530 @@
+// hydro_api.cu -- the C-ABI of include/hydro.h over the sm_100a kernels.
+// Host-side driver of Algorithm 1: persistent device state, one stream,
+// no per-step host<->device traffic except the 8-byte max-signal-speed read when the host
+// supplies dt (hydro_cfl_dt / hydro_evolve).
+#include "../../include/hydro.h"
+#include "hydro_kernels.cuh"
+#include "hydro_stage_fused.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+using namespace hyd;
+
+namespace {
+
+thread_local char g_err[512] = "";
+std::atomic<long long> g_launches{0};
+
+void *(*g_alloc)(size_t, void *) = nullptr;
+void (*g_release)(void *) = nullptr;
+
+int fail(int code, const char *fmt, const char *a = "", const char *b = "")
+{
+    snprintf(g_err, sizeof g_err, fmt, a, b);
+    return code;
+}
+
+#define CUDA_TRY(expr)                                                                   \
+    do {                                                                                 \
+        cudaError_t e_ = (expr);                                                         \
+        if (e_ != cudaSuccess)                                                           \
+            return fail(HYDRO_ERR_CUDA, "%s: %s", #expr, cudaGetErrorString(e_));        \
+    } while (0)
+
+#define LAUNCH_CHECK(name)                                                               \
+    do {                                                                                 \
+        g_launches.fetch_add(1, std::memory_order_relaxed);                              \
+        cudaError_t e_ = cudaGetLastError();                                             \
+        if (e_ != cudaSuccess)                                                           \
+            return fail(HYDRO_ERR_CUDA, "launch %s: %s", name, cudaGetErrorString(e_));  \
+    } while (0)
+
+}  // namespace
+
+struct hydro {
+    Grid g;
+    double dx, cfl;
+    double *block = nullptr;        // one allocation: [A | B]
+    double *A = nullptr, *B = nullptr;   // element (0,0,0) of variable 0 of each buffer
+    size_t buf_doubles = 0;         // doubles per buffer incl. lead
+    StepScalars *scal = nullptr;    // device scalars
+    StepScalars *scal_host = nullptr;   // pinned mirror for small reads
+    cudaStream_t stream = nullptr;
+    bool own_alloc_default = true;  // allocated through cudaMalloc (vs the hook)
+    void (*release)(void *) = nullptr;
+    bool have_state = false;
+    bool smax_valid = false;        // scal->smax_bits holds max(|v|+c) of the current state
+    bool t_on_device = false;       // run_steps advanced the device clock
+    double t = 0.0;
+    long long step = 0;
+    int variant = 0;
+    FusedPlan plan;                 // launch geometry / TMA descriptors of the fused kernel
+    // measurement hooks (hydro_set_profiling)
+    bool profiling = false;
+    struct Span { int which; cudaEvent_t a, b; };
+    std::vector<Span> spans;
+    std::vector<cudaEvent_t> pool;
+};
+
+namespace {
+
+constexpr int LEAD = 14;            // doubles before (0,0,0): first active cell of a row is 128-B aligned
+
+enum { K_GHOST = 0, K_STAGE1 = 1, K_STAGE2 = 2, K_NEXTDT = 3, K_CFL = 4 };
+
+cudaEvent_t take_event(hydro *h)
+{
+    cudaEvent_t e;
+    if (!h->pool.empty()) { e = h->pool.back(); h->pool.pop_back(); return e; }
+    cudaEventCreate(&e);
+    return e;
+}
+
+// Brackets one kernel launch with events on the handle's stream while profiling is on.
+struct Scope {
+    hydro *h; int which; cudaEvent_t a = nullptr;
+    Scope(hydro *h_, int w) : h(h_), which(w)
+    {
+        if (h->profiling) { a = take_event(h); cudaEventRecord(a, h->stream); }
+    }
+    ~Scope()
+    {
+        if (a) { cudaEvent_t b = take_event(h); cudaEventRecord(b, h->stream); h->spans.push_back({which, a, b}); }
+    }
+};
+
+int dev_alloc(hydro *h, void **p, size_t bytes)
+{
+    if (g_alloc) {
+        *p = g_alloc(bytes, (void *)h->stream);
+        h->own_alloc_default = false;
+        h->release = g_release;
+        return *p ? HYDRO_OK : fail(HYDRO_ERR_ALLOC, "allocator hook returned NULL%s%s");
+    }
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        *p = nullptr;
+        return fail(HYDRO_ERR_ALLOC, "cudaMalloc: %s%s", cudaGetErrorString(e));
+    }
+    return HYDRO_OK;
+}
+
+void dev_free(hydro *h, void *p)
+{
+    if (!p) return;
+    if (h->release) h->release(p);
+    else cudaFree(p);
+}
+
+int is_device_pointer(const void *p, bool *on_device)
+{
+    cudaPointerAttributes a;
+    cudaError_t e = cudaPointerGetAttributes(&a, p);
+    if (e != cudaSuccess) { cudaGetLastError(); *on_device = false; return HYDRO_OK; }
+    *on_device = (a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged);
+    return HYDRO_OK;
+}
+
+int launch_ghost_fill(hydro *h, double *U, bool clear_smax)
+{
+    const Grid &g = h->g;
+    const long long n = (long long)g.nx * g.ny + (long long)g.ny * g.nz + (long long)g.nz * g.nx;
+    const int tb = 128;
+    Scope sc(h, K_GHOST);
+    ghost_fill_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, h->stream>>>(
+        g, U, clear_smax ? &h->scal->smax_bits : nullptr);
+    LAUNCH_CHECK("ghost_fill");
+    return HYDRO_OK;
+}
+
+int launch_cfl_reduce(hydro *h)
+{
+    CUDA_TRY(cudaMemsetAsync(&h->scal->smax_bits, 0, sizeof(unsigned long long), h->stream));
+    const long long rows = (long long)h->g.ny * h->g.nz;
+    long long blocks = (rows + 7) / 8;
+    if (blocks > 148 * 8) blocks = 148 * 8;
+    Scope sc(h, K_CFL);
+    cfl_reduce_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->A, &h->scal->smax_bits,
+                                                               &h->scal->flag);
+    LAUNCH_CHECK("cfl_reduce");
+    h->smax_valid = true;
+    return HYDRO_OK;
+}
+
+template <int STAGE>
+int launch_stage(hydro *h, const double *in, const double *old, double *out, double r,
+                 bool dev_dt, bool reduce)
+{
+    const Grid &g = h->g;
+    const StepScalars *dd = dev_dt ? h->scal : nullptr;
+    StepScalars *red = reduce ? h->scal : nullptr;
+    Scope sc(h, STAGE == 1 ? K_STAGE1 : K_STAGE2);
+    if (h->variant == 0) {
+        dim3 tb(32, 4, 1);
+        dim3 gr((g.nx + 31) / 32, (g.ny + 3) / 4, g.nz);
+        stage_simple_kernel<STAGE><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
+        LAUNCH_CHECK("stage_simple");
+        return HYDRO_OK;
+    }
+    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, h->stream);
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused: %s%s", cudaGetErrorString(e));
+    return HYDRO_OK;
+}
+
+// One RK2 step (Algorithm 1 lines 6-21).  dt_host is ignored when dev_dt.
+int enqueue_step(hydro *h, double dt_host, bool dev_dt)
+{
+    const double r = dt_host / h->dx;
+    int rc;
+    if ((rc = launch_ghost_fill(h, h->A, false))) return rc;
+    if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
+    if ((rc = launch_ghost_fill(h, h->B, true))) return rc;
+    if ((rc = launch_stage<2>(h, h->B, h->A, h->A, r, dev_dt, true))) return rc;
+    h->smax_valid = true;
+    return HYDRO_OK;
+}
+
+int read_scalars(hydro *h)
+{
+    CUDA_TRY(cudaMemcpyAsync(h->scal_host, h->scal, sizeof(StepScalars), cudaMemcpyDeviceToHost,
+                             h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (h->t_on_device) {
+        h->t = h->scal_host->t;
+        h->step += h->scal_host->steps;
+        h->t_on_device = false;
+    }
+    return HYDRO_OK;
+}
+
+int copy_state(hydro *h, double *padded, double *packed, bool to_padded)
+{
+    const Grid &g = h->g;
+    bool dev;
+    is_device_pointer(packed, &dev);
+    if (dev) {
+        const long long nact = (long long)g.nx * g.ny * g.nz;
+        long long blocks = (nact + 255) / 256;
+        if (blocks > 148 * 16) blocks = 148 * 16;
+        if (to_padded) repack_kernel<true><<<(unsigned)blocks, 256, 0, h->stream>>>(g, padded, packed);
+        else repack_kernel<false><<<(unsigned)blocks, 256, 0, h->stream>>>(g, padded, packed);
+        LAUNCH_CHECK("repack");
+        return HYDRO_OK;
+    }
+    // host pointer: one pitched 3-D copy per variable straight into / out of the padded interior
+    for (int v = 0; v < NVAR; ++v) {
+        cudaMemcpy3DParms p;
+        memset(&p, 0, sizeof p);
+        cudaPitchedPtr dp = make_cudaPitchedPtr(padded + v * g.sv, (size_t)g.px * sizeof(double),
+                                                (size_t)g.px, (size_t)g.ny + 4);
+        cudaPitchedPtr hp = make_cudaPitchedPtr(packed + (size_t)v * g.nx * g.ny * g.nz,
+                                                (size_t)g.nx * sizeof(double), (size_t)g.nx,
+                                                (size_t)g.ny);
+        const cudaPos dpos = make_cudaPos(NG * sizeof(double), NG, NG);
+        const cudaPos hpos = make_cudaPos(0, 0, 0);
+        if (to_padded) { p.srcPtr = hp; p.srcPos = hpos; p.dstPtr = dp; p.dstPos = dpos; }
+        else           { p.srcPtr = dp; p.srcPos = dpos; p.dstPtr = hp; p.dstPos = hpos; }
+        p.extent = make_cudaExtent((size_t)g.nx * sizeof(double), (size_t)g.ny, (size_t)g.nz);
+        p.kind = to_padded ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToHost;
+        CUDA_TRY(cudaMemcpy3DAsync(&p, h->stream));
+    }
+    return HYDRO_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *hydro_last_error(void) { return g_err; }
+long long hydro_launch_count(void) { return g_launches.load(); }
+
+int hydro_is_verification_build(void)
+{
+#ifdef HYDRO_VERIFY
+    return 1;
+#else
+    return 0;
+#endif
+}
+
+int hydro_set_profiling(hydro_t *h, int enable)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "set_profiling: NULL handle%s%s");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    for (auto &s : h->spans) { h->pool.push_back(s.a); h->pool.push_back(s.b); }
+    h->spans.clear();
+    h->profiling = enable != 0;
+    return HYDRO_OK;
+}
+
+int hydro_get_kernel_time(hydro_t *h, int which, double *ms, long long *count)
+{
+    if (!h || !ms || !count) return fail(HYDRO_ERR_ARG, "get_kernel_time: NULL argument%s%s");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    double total = 0.0;
+    long long n = 0;
+    for (auto &s : h->spans)
+        if (s.which == which) {
+            float t = 0.f;
+            CUDA_TRY(cudaEventElapsedTime(&t, s.a, s.b));
+            total += t;
+            ++n;
+        }
+    *ms = total;
+    *count = n;
+    return HYDRO_OK;
+}
+
+int hydro_set_allocator(void *(*alloc)(size_t, void *), void (*release)(void *))
+{
+    if ((alloc == nullptr) != (release == nullptr))
+        return fail(HYDRO_ERR_ARG, "set_allocator: pass both hooks or neither%s%s");
+    g_alloc = alloc;
+    g_release = release;
+    return HYDRO_OK;
+}
+
+int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6], hydro_t **out)
+{
+    if (!out) return fail(HYDRO_ERR_ARG, "create: out is NULL%s%s");
+    *out = nullptr;
+    if (!bc) return fail(HYDRO_ERR_ARG, "create: bc is NULL%s%s");
+    if (nx < 2 || ny < 2 || nz < 2) return fail(HYDRO_ERR_ARG, "create: nx,ny,nz must be >= 2%s%s");
+    if (!(gamma > 1.0) || !std::isfinite(gamma)) return fail(HYDRO_ERR_ARG, "create: gamma must be > 1%s%s");
+    if (!(dx > 0.0) || !std::isfinite(dx)) return fail(HYDRO_ERR_ARG, "create: dx must be > 0%s%s");
+    for (int f = 0; f < 6; ++f)
+        if (bc[f] < 0 || bc[f] > 2) return fail(HYDRO_ERR_ARG, "create: unknown boundary kind%s%s");
+    for (int a = 0; a < 3; ++a)
+        if ((bc[2 * a] == HYDRO_BC_PERIODIC) != (bc[2 * a + 1] == HYDRO_BC_PERIODIC))
+            return fail(HYDRO_ERR_ARG, "create: periodic must be set on both faces of an axis%s%s");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(HYDRO_ERR_CUDA, "create: no CUDA device (there is no CPU fallback)%s%s");
+    }
+    hydro *h = new (std::nothrow) hydro;
+    if (!h) return fail(HYDRO_ERR_ALLOC, "create: host allocation failed%s%s");
+    Grid &g = h->g;
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    g.px = ((nx + 2 * NG + 15) / 16) * 16;
+    g.sy = (long long)g.px * (ny + 2 * NG);
+    const long long vol = g.sy * (nz + 2 * NG);
+    g.sv = ((vol + 15) / 16) * 16;
+    memcpy(g.bc, bc, sizeof g.bc);
+    g.gamma = gamma; g.gm1 = gamma - 1.0; g.igm1 = 1.0 / g.gm1; g.theta = 1.4; g.r_dx = 0.0;
+    h->dx = dx; h->cfl = 0.7;
+    // +16 tail so vectorised / TMA reads that run a few doubles past the last row stay inside
+    h->buf_doubles = (size_t)LEAD + (size_t)NVAR * g.sv + 16 + 2;
+    h->buf_doubles = ((h->buf_doubles + 15) / 16) * 16;
+    void *p = nullptr;
+    int rc = dev_alloc(h, &p, 2 * h->buf_doubles * sizeof(double));
+    if (rc) { delete h; return rc; }
+    h->block = (double *)p;
+    h->A = h->block + LEAD;
+    h->B = h->block + h->buf_doubles + LEAD;
+    cudaError_t e = cudaMalloc((void **)&h->scal, sizeof(StepScalars));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&h->scal_host, sizeof(StepScalars));
+    if (e == cudaSuccess) e = cudaMemset(h->block, 0, 2 * h->buf_doubles * sizeof(double));
+    if (e == cudaSuccess) e = cudaMemset(h->scal, 0, sizeof(StepScalars));
+    if (e == cudaSuccess) e = plan_stage_fused(h->plan, g, h->A, h->B);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        fail(HYDRO_ERR_CUDA, "create: %s%s", cudaGetErrorString(e));
+        hydro_destroy(h);
+        return HYDRO_ERR_CUDA;
+    }
+    *out = h;
+    return HYDRO_OK;
+}
+
+int hydro_destroy(hydro_t *h)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "destroy: NULL handle%s%s");
+    cudaStreamSynchronize(h->stream);
+    for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+    for (auto e : h->pool) cudaEventDestroy(e);
+    dev_free(h, h->block);
+    if (h->scal) cudaFree(h->scal);
+    if (h->scal_host) cudaFreeHost(h->scal_host);
+    delete h;
+    return HYDRO_OK;
+}
+
+int hydro_set_stream(hydro_t *h, void *s)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "set_stream: NULL handle%s%s");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    h->stream = (cudaStream_t)s;
+    return HYDRO_OK;
+}
+
+int hydro_set_cfl(hydro_t *h, double cfl)
+{
+    if (!h || !(cfl > 0.0) || !std::isfinite(cfl)) return fail(HYDRO_ERR_ARG, "set_cfl: cfl must be > 0%s%s");
+    h->cfl = cfl;
+    return HYDRO_OK;
+}
+
+int hydro_set_limiter_theta(hydro_t *h, double theta)
+{
+    if (!h || !(theta >= 1.0 && theta <= 2.0))
+        return fail(HYDRO_ERR_ARG, "set_limiter_theta: theta must be in [1,2]%s%s");
+    h->g.theta = theta;
+    return HYDRO_OK;
+}
+
+int hydro_set_kernel_variant(hydro_t *h, int variant)
+{
+    if (!h || variant < 0 || variant > 1) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0 or 1%s%s");
+    h->variant = variant;
+    return HYDRO_OK;
+}
+
+int hydro_set_state(hydro_t *h, const double *U)
+{
+    if (!h || !U) return fail(HYDRO_ERR_ARG, "set_state: NULL argument%s%s");
+    int rc = copy_state(h, h->A, const_cast<double *>(U), true);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemsetAsync(h->scal, 0, sizeof(StepScalars), h->stream));
+    bool dev;
+    is_device_pointer(U, &dev);
+    if (!dev) CUDA_TRY(cudaStreamSynchronize(h->stream));   // caller may free U on return
+    h->t = 0.0; h->step = 0; h->have_state = true; h->smax_valid = false; h->t_on_device = false;
+    return HYDRO_OK;
+}
+
+int hydro_get_state(hydro_t *h, double *U)
+{
+    if (!h || !U) return fail(HYDRO_ERR_ARG, "get_state: NULL argument%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "get_state before set_state%s%s");
+    int rc = copy_state(h, h->A, U, false);
+    if (rc) return rc;
+    if ((rc = read_scalars(h))) return rc;
+    if (h->scal_host->flag) return fail(HYDRO_ERR_UNPHYSICAL, "unphysical state (rho<=0, p<=0 or non-finite speed)%s%s");
+    return HYDRO_OK;
+}
+
+int hydro_ghost_fill(hydro_t *h)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "ghost_fill: NULL handle%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "ghost_fill before set_state%s%s");
+    return launch_ghost_fill(h, h->A, false);
+}
+
+int hydro_get_padded(hydro_t *h, double *Upad)
+{
+    if (!h || !Upad) return fail(HYDRO_ERR_ARG, "get_padded: NULL argument%s%s");
+    const Grid &g = h->g;
+    const size_t Nx = g.nx + 4, Ny = g.ny + 4, Nz = g.nz + 4;
+    for (int v = 0; v < NVAR; ++v)
+        for (size_t K = 0; K < Nz; ++K)
+            CUDA_TRY(cudaMemcpy2DAsync(Upad + ((size_t)v * Nz + K) * Ny * Nx, Nx * sizeof(double),
+                                       h->A + v * g.sv + K * g.sy, (size_t)g.px * sizeof(double),
+                                       Nx * sizeof(double), Ny, cudaMemcpyDefault, h->stream));
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    return HYDRO_OK;
+}
+
+int hydro_max_signal_speed(hydro_t *h, double *smax)
+{
+    if (!h || !smax) return fail(HYDRO_ERR_ARG, "max_signal_speed: NULL argument%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "max_signal_speed before set_state%s%s");
+    int rc;
+    if (!h->smax_valid && (rc = launch_cfl_reduce(h))) return rc;
+    if ((rc = read_scalars(h))) return rc;
+    double s;
+    memcpy(&s, &h->scal_host->smax_bits, sizeof s);
+    *smax = s;
+    if (h->scal_host->flag) return fail(HYDRO_ERR_UNPHYSICAL, "unphysical state (rho<=0, p<=0 or non-finite speed)%s%s");
+    return HYDRO_OK;
+}
+
+int hydro_cfl_dt(hydro_t *h, double *dt)
+{
+    if (!dt) return fail(HYDRO_ERR_ARG, "cfl_dt: NULL argument%s%s");
+    double smax;
+    int rc = hydro_max_signal_speed(h, &smax);
+    if (rc) return rc;
+    const double c3 = h->cfl / 3.0;
+    const double dxs = h->dx / smax;
+    *dt = c3 * dxs;
+    return HYDRO_OK;
+}
+
+int hydro_step(hydro_t *h, double dt)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "step: NULL handle%s%s");
+    if (!(dt > 0.0) || !std::isfinite(dt)) return fail(HYDRO_ERR_ARG, "step: dt must be > 0 and finite%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "step before set_state%s%s");
+    int rc;
+    if (h->t_on_device && (rc = read_scalars(h))) return rc;
+    if ((rc = enqueue_step(h, dt, false))) return rc;
+    h->t = h->t + dt;
+    h->step += 1;
+    return HYDRO_OK;
+}
+
+int hydro_run_steps(hydro_t *h, long long n)
+{
+    if (!h || n < 0) return fail(HYDRO_ERR_ARG, "run_steps: bad argument%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "run_steps before set_state%s%s");
+    if (n == 0) return HYDRO_OK;
+    int rc;
+    if (!h->smax_valid && (rc = launch_cfl_reduce(h))) return rc;
+    if (!h->t_on_device) {
+        begin_run_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->t);
+        LAUNCH_CHECK("begin_run");
+        h->t_on_device = true;
+    }
+    for (long long s = 0; s < n; ++s) {
+        {
+            Scope sc(h, K_NEXTDT);
+            next_dt_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->cfl, h->dx);
+        }
+        LAUNCH_CHECK("next_dt");
+        if ((rc = enqueue_step(h, 0.0, true))) return rc;
+    }
+    return HYDRO_OK;
+}
+
+int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
+{
+    if (!h || !std::isfinite(t_final)) return fail(HYDRO_ERR_ARG, "evolve: bad argument%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "evolve before set_state%s%s");
+    int rc;
+    if (h->t_on_device && (rc = read_scalars(h))) return rc;
+    if (t_final < h->t) return fail(HYDRO_ERR_ARG, "evolve: t_final is in the past%s%s");
+    long long n = 0;
+    while (h->t < t_final) {
+        double dt;
+        if ((rc = hydro_cfl_dt(h, &dt))) return rc;
+        bool last = false;
+        if (h->t + dt >= t_final) { dt = t_final - h->t; last = true; }
+        if ((rc = hydro_step(h, dt))) return rc;
+        if (last) h->t = t_final;
+        ++n;
+    }
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    if (nsteps) *nsteps = n;
+    return HYDRO_OK;
+}
+
+int hydro_get_time(hydro_t *h, double *t, long long *step)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "get_time: NULL handle%s%s");
+    int rc;
+    if (h->t_on_device && (rc = read_scalars(h))) return rc;
+    if (t) *t = h->t;
+    if (step) *step = h->step;
+    return HYDRO_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,280 @@
+// hydro_kernels.cuh -- sm_100a kernels of the RK2 Euler step: ghost fill (A1), stage kernels
+// (A2-A7), CFL reduction (A8), time-step bookkeeping.  See DESIGN.md section 5 for the layout and
+// section 6 for each kernel's roofline.
+#pragma once
+#include "hydro_math.cuh"
+
+namespace hyd {
+
+// Padded SoA state (A0): U[v][K][J][I], I fastest, row pitch `px` doubles (multiple of 16),
+// active cells I in [2, nx+1] etc.  `lead` doubles precede element (0,0,0) of every variable so
+// that the first active cell of every row sits on a 128-byte boundary.
+struct Grid {
+    int nx, ny, nz;          // active cells
+    int px;                  // row pitch (doubles)
+    long long sy;            // plane stride = px * (ny+4)
+    long long sv;            // variable stride (doubles), multiple of 16
+    int bc[6];
+    double gamma, gm1, igm1, theta;
+    double r_dx;             // unused by kernels that take dt/dx directly
+};
+
+__device__ __forceinline__ long long cell(const Grid &g, int I, int J, int K)
+{
+    return (long long)I + (long long)g.px * J + g.sy * K;
+}
+
+// ------------------------------------------------------------------------------------------
+// A1 ghost fill (R9).  One thread per (face pair of one axis, transverse active cell); each
+// thread fills the 2+2 ghost cells of its line for all 5 variables.  The three axes are
+// independent because only active transverse indices are filled.
+// Thread 0 optionally clears the max-signal-speed accumulator for the stage that follows.
+// ------------------------------------------------------------------------------------------
+__global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
+                                  unsigned long long *__restrict__ clear_smax)
+{
+    const long long nxy = (long long)g.nx * g.ny, nyz = (long long)g.ny * g.nz,
+                    nzx = (long long)g.nz * g.nx;
+    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t == 0 && clear_smax) *clear_smax = 0ull;
+    int axis, n;
+    long long base, stride;
+    if (t < nxy) {                       // z faces: thread per (i,j), coalesced in i
+        const int i = (int)(t % g.nx), j = (int)(t / g.nx);
+        axis = 2; n = g.nz; base = cell(g, i + NG, j + NG, 0); stride = g.sy;
+    } else if ((t -= nxy) < nzx) {       // y faces: thread per (i,k), coalesced in i
+        const int i = (int)(t % g.nx), k = (int)(t / g.nx);
+        axis = 1; n = g.ny; base = cell(g, i + NG, 0, k + NG); stride = g.px;
+    } else if ((t -= nzx) < nyz) {       // x faces: thread per (j,k)
+        const int j = (int)(t % g.ny), k = (int)(t / g.ny);
+        axis = 0; n = g.nx; base = cell(g, 0, j + NG, k + NG); stride = 1;
+    } else {
+        return;
+    }
+    const int lo = g.bc[2 * axis], hi = g.bc[2 * axis + 1];
+#pragma unroll
+    for (int v = 0; v < NVAR; ++v) {
+        double *a = U + v * g.sv + base;
+        const double sgn = (v == 1 + axis) ? -1.0 : 1.0;
+        // sources are always active cells [2, n+1]
+        const double a2 = a[2 * stride], a3 = a[3 * stride];
+        const double an = a[(long long)n * stride], an1 = a[(long long)(n + 1) * stride];
+        double g0, g1, g2, g3;
+        if (lo == 0)      { g0 = a2; g1 = a2; }
+        else if (lo == 1) { g0 = sgn * a3; g1 = sgn * a2; }
+        else              { g0 = an; g1 = an1; }
+        if (hi == 0)      { g2 = an1; g3 = an1; }
+        else if (hi == 1) { g2 = sgn * an1; g3 = sgn * an; }
+        else              { g2 = a2; g3 = a3; }
+        a[0] = g0; a[stride] = g1;
+        a[(long long)(n + 2) * stride] = g2; a[(long long)(n + 3) * stride] = g3;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// A8 stand-alone CFL reduction: smax = max over active cells of |v| + c_s (O7), as an integer
+// atomicMax on the bit pattern (non-negative doubles order like their bit patterns), plus a
+// sticky flag for unphysical cells (R12).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void block_max_to_global(double s, int bad,
+                                                    unsigned long long *smax_bits, int *flag)
+{
+    // NaN never wins a '>' comparison; it is reported through `bad` instead
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double other = __shfl_xor_sync(0xffffffffu, s, o);
+        s = other > s ? other : s;
+        bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    __shared__ double wmax[32];
+    __shared__ int wbad[32];
+    const int tid = threadIdx.x + blockDim.x * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int lane = tid & 31, wid = tid >> 5;
+    const int nw = (blockDim.x * blockDim.y * blockDim.z + 31) >> 5;
+    if (lane == 0) { wmax[wid] = s; wbad[wid] = bad; }
+    __syncthreads();
+    if (wid == 0) {
+        s = lane < nw ? wmax[lane] : 0.0;
+        bad = lane < nw ? wbad[lane] : 0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double other = __shfl_xor_sync(0xffffffffu, s, o);
+            s = other > s ? other : s;
+            bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+        }
+        if (lane == 0) {
+            if (s > 0.0) atomicMax(smax_bits, (unsigned long long)__double_as_longlong(s));
+            if (bad) atomicOr(flag, 1);
+        }
+    }
+}
+
+__device__ __forceinline__ double cell_signal_speed(double rho, double mx, double my, double mz,
+                                                    double E, double gamma, double gm1, int &bad)
+{
+    double inv, q;
+    const Prim w = primitive(rho, mx, my, mz, E, gm1, inv, q);
+    const double s = signal_speed(w, inv, q, gamma);
+    if (!(rho > 0.0) || !(w.p > 0.0) || !(s <= 1.79769313486231570e308)) bad = 1;
+    return s;
+}
+
+__global__ void __launch_bounds__(256)
+cfl_reduce_kernel(Grid g, const double *__restrict__ U, unsigned long long *smax_bits, int *flag)
+{
+    double s = 0.0;
+    int bad = 0;
+    const long long nrow = (long long)g.ny * g.nz;
+    // one warp per x-row at a time: coalesced, grid-stride over rows
+    const int lane = threadIdx.x & 31;
+    const long long wglobal = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long row = wglobal; row < nrow; row += nwarps) {
+        const int j = (int)(row % g.ny), k = (int)(row / g.ny);
+        const double *u = U + cell(g, NG, j + NG, k + NG);
+        for (int i = lane; i < g.nx; i += 32) {
+            const double c = cell_signal_speed(u[i], u[g.sv + i], u[2 * g.sv + i], u[3 * g.sv + i],
+                                               u[4 * g.sv + i], g.gamma, g.gm1, bad);
+            s = c > s ? c : s;
+        }
+    }
+    block_max_to_global(s, bad, smax_bits, flag);
+}
+
+// Device-resident time step (hydro_run_steps): dt = (cfl/3) * (dx / smax); t += dt.
+struct StepScalars {
+    unsigned long long smax_bits;   // running max of the CFL reduction (bit pattern)
+    int flag;                       // sticky: unphysical state seen
+    int pad;
+    double dt;                      // time step of the current step
+    double t;                       // simulation time (device copy, used by run_steps)
+    long long steps;                // steps taken by run_steps since begin
+};
+
+__global__ void begin_run_kernel(StepScalars *s, double t0)
+{
+    s->t = t0;
+    s->steps = 0;
+}
+
+__global__ void next_dt_kernel(StepScalars *s, double cfl, double dx)
+{
+    const double smax = __longlong_as_double((long long)s->smax_bits);
+    const double c3 = cfl / 3.0;
+    const double dxs = dx / smax;
+    const double dt = c3 * dxs;
+    s->dt = dt;
+    s->t = s->t + dt;
+    s->steps += 1;
+}
+
+// ------------------------------------------------------------------------------------------
+// Stage kernel, variant 0 ("simple"): one thread per active cell, global loads through L1/L2,
+// every slope and face the cell needs recomputed by the thread itself (13-cell stencil).
+// Same arithmetic as the fused kernel; kept as the bring-up and cross-check implementation.
+// STAGE 1: out = U0 + dU(U0).   STAGE 2: out = 0.5*((U0 + U1) + dU(U1)) (+ fused CFL max).
+// ------------------------------------------------------------------------------------------
+template <int D>
+__device__ __forceinline__ void load_prim_line(const Grid &g, const double *__restrict__ U,
+                                               long long c, long long stride, double W[5][5])
+{
+    // W[o][.] = primitives of the cell at offset o-2 along D, in (rho, n, t1, t2, p) order
+#pragma unroll
+    for (int o = 0; o < 5; ++o) {
+        const long long cc = c + (o - 2) * stride;
+        const Prim w = primitive(__ldg(U + cc), __ldg(U + g.sv + cc), __ldg(U + 2 * g.sv + cc),
+                                 __ldg(U + 3 * g.sv + cc), __ldg(U + 4 * g.sv + cc), g.gm1);
+        const double v[3] = { w.vx, w.vy, w.vz };
+        W[o][0] = w.rho; W[o][1] = v[D]; W[o][2] = v[(D + 1) % 3]; W[o][3] = v[(D + 2) % 3];
+        W[o][4] = w.p;
+    }
+}
+
+template <int D>
+__device__ __forceinline__ void flux_difference(const Grid &g, const double *__restrict__ U,
+                                                long long c, long long stride, double dF[5])
+{
+    double W[5][5];
+    load_prim_line<D>(g, U, c, stride, W);
+    double Lm[5], Rm[5], Lp[5], Rp[5];     // faces i-1/2 and i+1/2
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        const double sm = minmod(g.theta, W[1][v] - W[0][v], W[2][v] - W[1][v]);
+        const double s0 = minmod(g.theta, W[2][v] - W[1][v], W[3][v] - W[2][v]);
+        const double sp = minmod(g.theta, W[3][v] - W[2][v], W[4][v] - W[3][v]);
+        Lm[v] = W[1][v] + 0.5 * sm;      // outer(i-1)
+        Rm[v] = W[2][v] - 0.5 * s0;      // inner(i)
+        Lp[v] = W[2][v] + 0.5 * s0;      // outer(i)
+        Rp[v] = W[3][v] - 0.5 * sp;      // inner(i+1)
+    }
+    double Fm[5], Fp[5];
+    hll_flux(Lm, Rm, g.gamma, g.igm1, Fm);
+    hll_flux(Lp, Rp, g.gamma, g.igm1, Fp);
+    // (rho, n, t1, t2, E) -> (rho, mx, my, mz, E)
+    dF[0] = Fp[0] - Fm[0];
+    dF[1 + D] = Fp[1] - Fm[1];
+    dF[1 + (D + 1) % 3] = Fp[2] - Fm[2];
+    dF[1 + (D + 2) % 3] = Fp[3] - Fm[3];
+    dF[4] = Fp[4] - Fm[4];
+}
+
+template <int STAGE>
+__global__ void __launch_bounds__(128)
+stage_simple_kernel(Grid g, const double *__restrict__ Uin, const double *Uold, double *Uout,
+                    double dt_over_dx, const StepScalars *__restrict__ dev_dt, double dx,
+                    StepScalars *__restrict__ red)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = blockIdx.z;
+    double s = 0.0;
+    int bad = 0;
+    if (i < g.nx && j < g.ny) {
+        const double r = dev_dt ? dev_dt->dt / dx : dt_over_dx;
+        const long long c = cell(g, i + NG, j + NG, k + NG);
+        double dFx[5], dFy[5], dFz[5];
+        flux_difference<0>(g, Uin, c, 1, dFx);
+        flux_difference<1>(g, Uin, c, g.px, dFy);
+        flux_difference<2>(g, Uin, c, g.sy, dFz);
+        double un[5];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) {
+            const double D = sum3(dFx[v], dFy[v], dFz[v]);
+            const double dU = -(r * D);
+            if (STAGE == 1) {
+                un[v] = Uin[v * g.sv + c] + dU;
+            } else {
+                const double sum = Uold[v * g.sv + c] + Uin[v * g.sv + c];
+                un[v] = 0.5 * (sum + dU);
+            }
+            Uout[v * g.sv + c] = un[v];
+        }
+        if (STAGE == 2 && red)
+            s = cell_signal_speed(un[0], un[1], un[2], un[3], un[4], g.gamma, g.gm1, bad);
+    }
+    if (STAGE == 2 && red) block_max_to_global(s, bad, &red->smax_bits, &red->flag);
+}
+
+// ------------------------------------------------------------------------------------------
+// pack / unpack between the packed [5][nz][ny][nx] layout and the padded state (device side;
+// host pointers go through cudaMemcpy3D in the API layer).
+// ------------------------------------------------------------------------------------------
+template <bool TO_PADDED>
+__global__ void repack_kernel(Grid g, double *padded, double *packed)
+{
+    const long long nact = (long long)g.nx * g.ny * g.nz;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nact;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(t % g.nx);
+        const long long jk = t / g.nx;
+        const int j = (int)(jk % g.ny), k = (int)(jk / g.ny);
+        const long long c = cell(g, i + NG, j + NG, k + NG);
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) {
+            if (TO_PADDED) padded[v * g.sv + c] = packed[v * nact + t];
+            else packed[v * nact + t] = padded[v * g.sv + c];
+        }
+    }
+}
+
+}  // namespace hyd

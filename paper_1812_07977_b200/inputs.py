@@ -97,6 +97,7 @@ class Config:
     t_final: float = 0.0
     theta: float = 1.4
     make: object = field(default=None, repr=False)
+    index: int = -1
 
     @property
     def cells(self):
@@ -129,3 +130,13 @@ def config(i):
         return Config("cfg4_noise512", (512, 512, 512), 5.0 / 3.0, 0.5, _PER6, 1.0 / 512,
                       steps=50, make=lambda: noise(512))
     raise ValueError(i)
+
+
+_config_raw = config
+
+
+def config(i):  # noqa: F811
+    """BASELINE.json:configs[i] as a Config (with .index set)."""
+    c = _config_raw(i)
+    c.index = i
+    return c

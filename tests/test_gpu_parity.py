@@ -1,0 +1,404 @@
+"""GPU-vs-oracle parity through the C-ABI (all `-m gpu`).
+
+Bars (BASELINE.json:north_star):
+  * verification build (-fmad=false): |a-b| <= 1e-14 * max(|b|, S_v) per cell after one step
+    (S_v = max|b_v| over the grid, the three momenta sharing one scale); in practice bit-identical,
+    which is asserted where noted;
+  * production build: relL1 <= 1e-10 and relLinf <= 1e-8 per conserved variable at the end of each
+    config's run;
+  * integer/flag results (step counts, error codes, ghost cells) exact.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_1812_07977_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+OUT, REF, PER = 0, 1, 2
+DEFAULT_VARIANT = int(os.environ.get("HYDRO_VARIANT", "1"))
+VARIANTS = [0, 1] if DEFAULT_VARIANT == 1 else [0]
+
+
+def _mk(cls, shape, gamma, dx, bc, cfl=0.7, theta=None, **kw):
+    h = cls(*shape, gamma, dx, bc, **kw)
+    h.set_cfl(cfl)
+    if theta is not None:
+        h.set_limiter_theta(theta)
+    return h
+
+
+def _gpu(shape, gamma, dx, bc, cfl=0.7, theta=None, verify=False, variant=None):
+    variant = DEFAULT_VARIANT if variant is None else variant
+    from paper_1812_07977_b200.binding import Hydro
+    h = _mk(Hydro, shape, gamma, dx, bc, cfl, theta, verify=verify)
+    h.set_kernel_variant(variant)
+    return h
+
+
+def _cpu(shape, gamma, dx, bc, cfl=0.7, theta=None):
+    from oracle import OracleHydro
+    return _mk(OracleHydro, shape, gamma, dx, bc, cfl, theta)
+
+
+def scales(b):
+    s = np.array([np.abs(b[v]).max() for v in range(5)])
+    m = s[1:4].max()
+    if m == 0.0:
+        m = 1.0
+    s[1:4] = m
+    return s
+
+
+def assert_one_step_bar(a, b, tol=1e-14):
+    s = scales(b)
+    for v in range(5):
+        bound = tol * np.maximum(np.abs(b[v]), s[v])
+        bad = np.abs(a[v] - b[v]) > bound
+        assert not bad.any(), (v, int(bad.sum()), float(np.abs(a[v] - b[v]).max()))
+
+
+def rel_norms(a, b):
+    """(relL1, relLinf) per conserved variable, momenta sharing one scale, 0/0 := 0."""
+    l1d = np.array([np.abs(a[v] - b[v]).sum() for v in range(5)])
+    l1s = np.array([np.abs(b[v]).sum() for v in range(5)])
+    lid = np.array([np.abs(a[v] - b[v]).max() for v in range(5)])
+    lis = np.array([np.abs(b[v]).max() for v in range(5)])
+    l1s[1:4] = l1s[1:4].max()
+    lis[1:4] = lis[1:4].max()
+    with np.errstate(invalid="ignore", divide="ignore"):
+        r1 = np.where(l1d == 0, 0.0, l1d / l1s)
+        ri = np.where(lid == 0, 0.0, lid / lis)
+    return r1, ri
+
+
+def assert_production_bar(a, b):
+    r1, ri = rel_norms(a, b)
+    assert (r1 <= 1e-10).all() and (ri <= 1e-8).all(), (r1, ri)
+
+
+# ---------------------------------------------------------------- boundary kernels
+
+BCS = [(OUT,) * 6, (PER,) * 6, (REF,) * 6, (OUT, REF, PER, PER, REF, OUT),
+       (REF, OUT, REF, REF, PER, PER)]
+
+
+@pytest.mark.parametrize("bc", BCS)
+@pytest.mark.parametrize("shape", [(5, 4, 3), (37, 9, 6), (2, 2, 2)])
+def test_ghost_fill_bit_exact(bc, shape):
+    nx, ny, nz = shape
+    U = inputs.random_state(nx, ny, nz, seed=7)
+    g = _gpu(shape, 1.4, 0.1, bc)
+    c = _cpu(shape, 1.4, 0.1, bc)
+    g.set_state(U); c.set_state(U)
+    g.ghost_fill(); c.ghost_fill()
+    a, b = g.get_padded(), c.get_padded()
+    # compare active cells and the face slabs; edges/corners are don't-care (never read)
+    gz = np.zeros(nz + 4, bool); gz[:2] = gz[-2:] = True
+    gy = np.zeros(ny + 4, bool); gy[:2] = gy[-2:] = True
+    gx = np.zeros(nx + 4, bool); gx[:2] = gx[-2:] = True
+    nghost = gz[:, None, None].astype(int) + gy[None, :, None] + gx[None, None, :]
+    mask = np.broadcast_to(nghost <= 1, a.shape)
+    assert np.array_equal(a[mask], b[mask])
+
+
+def test_set_get_state_roundtrip_host_and_device():
+    import torch
+    shape = (19, 7, 5)
+    U = inputs.random_state(*shape, seed=3)
+    g = _gpu(shape, 1.4, 0.1, (OUT,) * 6)
+    g.set_state(U)
+    assert np.array_equal(g.get_state(), U)
+    Ud = torch.from_numpy(U).cuda()
+    g.set_state(Ud)
+    out = torch.empty_like(Ud)
+    g.get_state(out)
+    assert torch.equal(out, Ud)
+    pinned = torch.from_numpy(U).pin_memory()
+    g.set_state(pinned)
+    assert np.array_equal(g.get_state(), U)
+
+
+@pytest.mark.parametrize("shape", [(32, 32, 32), (45, 7, 3)])
+def test_cfl_reduction_bit_exact(shape):
+    U = inputs.random_state(*shape, seed=11)
+    for verify in (True, False):
+        g = _gpu(shape, 5 / 3, 0.05, (PER,) * 6, cfl=0.5, verify=verify)
+        c = _cpu(shape, 5 / 3, 0.05, (PER,) * 6, cfl=0.5)
+        g.set_state(U); c.set_state(U)
+        if verify:
+            assert g.max_signal_speed() == c.max_signal_speed()
+            assert g.cfl_dt() == c.cfl_dt()
+        else:
+            assert abs(g.max_signal_speed() - c.max_signal_speed()) <= 4e-16 * c.max_signal_speed()
+
+
+def test_config0_first_dt_matches_paper_recipe_value():
+    c = inputs.config(0)
+    g = _gpu(c.shape, c.gamma, c.dx, c.bc, c.cfl, verify=True)
+    g.set_state(c.state())
+    assert g.cfl_dt() == (0.7 / 3.0) * ((1.0 / 32.0) / np.sqrt(1.4))
+
+
+# ---------------------------------------------------------------- one step, verification build
+
+ONE_STEP_CASES = [
+    ((32, 32, 32), (OUT,) * 6, "sphere"),
+    ((37, 21, 9), (PER,) * 6, "random"),            # ragged: not multiples of any tile
+    ((70, 35, 12), (OUT, REF, PER, PER, REF, OUT), "random"),
+    ((16, 40, 33), (REF,) * 6, "random"),
+    ((2, 2, 2), (PER,) * 6, "random"),              # degenerate minimum
+    ((3, 2, 5), (OUT, OUT, REF, REF, PER, PER), "random"),
+    ((130, 6, 4), (OUT, OUT, PER, PER, PER, PER), "sod"),
+]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("shape,bc,kind", ONE_STEP_CASES)
+def test_one_step_verification_build_bit_identical(shape, bc, kind, variant):
+    nx, ny, nz = shape
+    if kind == "sphere":
+        U = inputs.sphere(nx)
+    elif kind == "sod":
+        U = inputs.sod(nx, ny, nz)
+    else:
+        U = inputs.random_state(nx, ny, nz, seed=nx + ny + nz, vamp=0.6)
+    g = _gpu(shape, 1.4, 1.0 / nx, bc, verify=True, variant=variant)
+    c = _cpu(shape, 1.4, 1.0 / nx, bc)
+    g.set_state(U); c.set_state(U)
+    dt = c.cfl_dt()
+    assert g.cfl_dt() == dt
+    g.step(dt); c.step(dt)
+    a, b = g.get_state(), c.get_state()
+    assert_one_step_bar(a, b)                      # the stated bar
+    assert np.array_equal(a, b)                    # what the -fmad=false build actually achieves
+    # fused CFL reduction of the new state
+    assert g.max_signal_speed() == c.max_signal_speed()
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_one_step_production_build_within_1e14(variant):
+    c0 = inputs.config(0)
+    U = c0.state()
+    g = _gpu(c0.shape, c0.gamma, c0.dx, c0.bc, c0.cfl, variant=variant)
+    c = _cpu(c0.shape, c0.gamma, c0.dx, c0.bc, c0.cfl)
+    g.set_state(U); c.set_state(U)
+    dt = c.cfl_dt()
+    g.step(dt); c.step(dt)
+    # FMA contraction changes roundings: a few ulp, far inside the production bar
+    assert_one_step_bar(g.get_state(), c.get_state(), tol=2e-14)
+
+
+# ---------------------------------------------------------------- end-of-run parity per config
+
+def _run_pair(cfg, U, verify, variant, steps=None, use_run_steps=False):
+    g = _gpu(cfg.shape, cfg.gamma, cfg.dx, cfg.bc, cfg.cfl, verify=verify, variant=variant)
+    c = _cpu(cfg.shape, cfg.gamma, cfg.dx, cfg.bc, cfg.cfl)
+    g.set_state(U); c.set_state(U)
+    n = cfg.steps if steps is None else steps
+    if cfg.t_final and steps is None:
+        ng, nc = g.evolve(cfg.t_final), c.evolve(cfg.t_final)
+        assert g.get_time()[0] == cfg.t_final == c.get_time()[0]
+        return g, c, ng, nc
+    if use_run_steps:
+        g.run_steps(n)
+    else:
+        for _ in range(n):
+            g.step(g.cfl_dt())
+    for _ in range(n):
+        c.step(c.cfl_dt())
+    return g, c, n, n
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_config0_twenty_steps(variant):
+    cfg = inputs.config(0)
+    U = cfg.state()
+    g, c, _, _ = _run_pair(cfg, U, True, variant)
+    assert np.array_equal(g.get_state(), c.get_state())          # verification build: bitwise
+    assert g.get_time() == c.get_time()
+    g, c, _, _ = _run_pair(cfg, U, False, variant)
+    assert_production_bar(g.get_state(), c.get_state())
+    g, c, _, _ = _run_pair(cfg, U, False, variant, use_run_steps=True)   # device-resident dt
+    assert_production_bar(g.get_state(), c.get_state())
+    tg, tc = g.get_time(), c.get_time()
+    assert tg[1] == tc[1] and abs(tg[0] - tc[0]) <= 1e-12 * tc[0]
+
+
+def test_run_steps_equals_host_loop_bitwise_on_verification_build():
+    cfg = inputs.config(0)
+    U = cfg.state()
+    g, c, _, _ = _run_pair(cfg, U, True, None, steps=7, use_run_steps=True)
+    assert np.array_equal(g.get_state(), c.get_state())
+    assert g.get_time() == c.get_time()
+
+
+def test_config1_sod_evolve_to_t02():
+    cfg = inputs.config(1)
+    U = cfg.state()
+    g, c, ng, nc = _run_pair(cfg, U, True, None)
+    assert ng == nc
+    assert np.array_equal(g.get_state(), c.get_state())
+    g, c, ng, nc = _run_pair(cfg, U, False, None)
+    assert abs(ng - nc) <= 1
+    a = g.get_state()
+    assert_production_bar(a, c.get_state())
+    # P2 addendum on the GPU result: rows identical, transverse momenta exactly zero
+    assert np.array_equal(a, np.broadcast_to(a[:, :1, :1, :], a.shape))
+    assert not a[2].any() and not a[3].any()
+
+
+def test_config2_sphere128_hundred_steps():
+    cfg = inputs.config(2)
+    U = cfg.state()
+    g, c, _, _ = _run_pair(cfg, U, False, None)
+    a = g.get_state()
+    assert_production_bar(a, c.get_state())
+    _assert_cubic_symmetry(a)
+
+
+def _assert_cubic_symmetry(a):
+    import itertools
+    for perm in itertools.permutations((0, 1, 2)):
+        assert np.array_equal(inputs.permute_axes(a, perm), a), perm
+    for ax in range(3):
+        assert np.array_equal(inputs.reflect_axis(a, ax), a), ax
+
+
+def test_config4_shape_noise_periodic_conservation_and_parity():
+    # config 4's recipe at an oracle-sized grid (96^3, several tiles + ragged tail in every axis)
+    n = 96
+    cfg = inputs.config(4)
+    cfg.shape, cfg.dx, cfg.steps = (n, n, n), 1.0 / n, 10
+    U = inputs.noise(n, seed=12345)
+    g, c, _, _ = _run_pair(cfg, U, False, None)
+    a = g.get_state()
+    assert_production_bar(a, c.get_state())
+    for v in (0, 4):
+        assert abs(a[v].sum() - U[v].sum()) <= 1e-13 * abs(U[v].sum())
+
+
+# ---------------------------------------------------------------- full-size checks (launch config of bench.py)
+
+def test_config3_full_size_sampled_and_symmetry():
+    """256^3 in the launch configuration bench.py times: 4 steps against the full oracle,
+    then the whole 200-step run checked through P4 (bitwise cubic symmetry) and positivity."""
+    cfg = inputs.config(3)
+    U = cfg.state()
+    g, c, _, _ = _run_pair(cfg, U, False, None, steps=4)
+    assert_production_bar(g.get_state(), c.get_state())
+    del c
+    g.run_steps(cfg.steps - 4)
+    a = g.get_state()
+    assert g.get_time()[1] == cfg.steps
+    _assert_cubic_symmetry(a)
+    assert a[0].min() == 0.125 and np.isfinite(a).all()
+
+
+@pytest.mark.skipif(os.environ.get("HYDRO_FULL_PARITY") != "1",
+                    reason="~10 min of oracle time; set HYDRO_FULL_PARITY=1")
+def test_config3_full_run_against_oracle():
+    cfg = inputs.config(3)
+    U = cfg.state()
+    g, c, _, _ = _run_pair(cfg, U, False, None)
+    assert_production_bar(g.get_state(), c.get_state())
+
+
+def test_config4_full_size_periodic_tiling_and_conservation():
+    """512^3: (i) a 64^3 noise block tiled 8x8x8 must evolve exactly like the 64^3 periodic
+    problem the oracle runs (P8: periodic images), every cell compared; (ii) config 4 itself
+    (iid noise, seed 12345) must conserve mass, momentum and energy to roundoff over 50 steps."""
+    import torch
+    cfg = inputs.config(4)
+    small = inputs.noise(64, seed=12345)
+    steps = 6
+    c = _cpu((64, 64, 64), cfg.gamma, cfg.dx, cfg.bc, cfg.cfl)
+    c.set_state(small)
+    dts = []
+    for _ in range(steps):
+        dts.append(c.cfl_dt()); c.step(dts[-1])
+    ref = c.get_state()
+    g = _gpu(cfg.shape, cfg.gamma, cfg.dx, cfg.bc, cfg.cfl, verify=True)
+    big = torch.from_numpy(small).cuda().repeat(1, 8, 8, 8).contiguous()
+    g.set_state(big)
+    for dt in dts:
+        assert g.cfl_dt() == dt
+        g.step(dt)
+    out = torch.empty_like(big)
+    g.get_state(out)
+    want = torch.from_numpy(ref).cuda().repeat(1, 8, 8, 8)
+    assert torch.equal(out, want)
+    del big, out, want
+    g.close()
+    # (ii) the real config 4
+    U = torch.from_numpy(cfg.state()).cuda()
+    sums0 = U.sum(dim=(1, 2, 3), dtype=torch.float64).cpu().numpy()
+    mscale = U[1:4].abs().sum().item()
+    g = _gpu(cfg.shape, cfg.gamma, cfg.dx, cfg.bc, cfg.cfl)
+    g.set_state(U)
+    g.run_steps(cfg.steps)
+    g.get_state(U)
+    sums1 = U.sum(dim=(1, 2, 3), dtype=torch.float64).cpu().numpy()
+    assert torch.isfinite(U).all()
+    for v in (0, 4):
+        assert abs(sums1[v] - sums0[v]) <= 1e-12 * abs(sums0[v])
+    for v in (1, 2, 3):
+        assert abs(sums1[v] - sums0[v]) <= 1e-12 * mscale
+
+
+# ---------------------------------------------------------------- errors and flags
+
+def test_unphysical_state_is_reported_by_the_fused_reduction():
+    from paper_1812_07977_b200.binding import HydroError
+    c0 = inputs.config(0)
+    g = _gpu(c0.shape, c0.gamma, c0.dx, c0.bc, c0.cfl)
+    g.set_state(c0.state())
+    dt = 0.7 * c0.dx / g.max_signal_speed()        # the literal CFL reading (R8) blows up
+    g.step(dt); g.step(dt)
+    with pytest.raises(HydroError) as e:
+        g.cfl_dt()
+    assert e.value.code == 4
+    g.set_state(c0.state())                        # set_state clears the sticky flag
+    assert g.cfl_dt() > 0
+
+
+def test_status_codes():
+    from paper_1812_07977_b200.binding import Hydro, HydroError
+    g = Hydro(4, 4, 4, 1.4, 0.1, (0,) * 6)
+    with pytest.raises(HydroError) as e:
+        g.step(0.1)
+    assert e.value.code == 5
+    g.set_state(inputs.random_state(4, 4, 4))
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(HydroError) as e:
+            g.step(bad)
+        assert e.value.code == 1
+    with pytest.raises(HydroError):
+        g.set_limiter_theta(0.5)
+    n0 = g.launch_count()
+    g.step(g.cfl_dt())
+    assert g.launch_count() >= n0 + 4
+
+
+def test_uniform_state_bit_identical_on_production_build():
+    ones = np.ones((9, 40, 70))
+    U = inputs.conserved_from_primitive(0.7 * ones, 0.31 * ones, -0.17 * ones, 0.53 * ones,
+                                        1.3 * ones, 1.4)
+    for variant in VARIANTS:
+        g = _gpu((70, 40, 9), 1.4, 0.1, (OUT, OUT, PER, PER, OUT, OUT), variant=variant)
+        g.set_state(U)
+        g.run_steps(5)
+        assert np.array_equal(g.get_state(), U)
+
+
+def test_deterministic_run_to_run():
+    U = inputs.noise(48, seed=5)
+    outs = []
+    for _ in range(2):
+        g = _gpu((48, 48, 48), 5 / 3, 1 / 48, (PER,) * 6, cfl=0.5)
+        g.set_state(U)
+        g.run_steps(8)
+        outs.append(g.get_state())
+    assert np.array_equal(outs[0], outs[1])
