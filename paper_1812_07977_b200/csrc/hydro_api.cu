@@ -62,7 +62,7 @@ struct hydro {
     bool t_on_device = false;       // run_steps advanced the device clock
     double t = 0.0;
     long long step = 0;
-    int variant = 0;
+    int variant = 1;
     FusedPlan plan;                 // launch geometry / TMA descriptors of the fused kernel
     // measurement hooks (hydro_set_profiling)
     bool profiling = false;

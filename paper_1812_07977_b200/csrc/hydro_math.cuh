@@ -109,7 +109,8 @@ __device__ __forceinline__ void hll_flux(const double L[5], const double R[5], d
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
         const double num = (ap * sl.F[v] + am * sr.F[v]) - pi * (sr.U[v] - sl.U[v]);
-        F[v] = num * w;
+        F[v] = __dmul_rn(num, w);   // never contracted into a consumer's subtract: equal
+                                    // face states must give bit-equal fluxes on every build (P1)
     }
 }
 

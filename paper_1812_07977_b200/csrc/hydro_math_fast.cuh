@@ -1,0 +1,120 @@
+// hydro_math_fast.cuh -- production-build arithmetic of the fused stage kernel.
+//
+// Same formulas as hydro_math.cuh (O2-O7) with the freedoms the production
+// build takes (R20 and section 6): FMA contraction, branch-free reciprocal / reciprocal
+// square root built on MUFU.RCP64H / MUFU.RSQ64H seeds plus Newton steps (<= 2 ulp instead of
+// correctly rounded), sign handling of the limiter on the integer pipe, plain (x+y)+z instead of
+// the sorted three-term sum.  Results differ from the oracle at roundoff only; the parity bar for
+// this build is relL1 <= 1e-10, relLinf <= 1e-8 (BASELINE.json:north_star).  The verification
+// build (-DHYDRO_VERIFY, -fmad=false) never includes this path.
+//
+// Why: the stage kernel is bound by the fp64 pipe and by issue slots, so
+// every DSETP/FSEL pair and every slow-path branch of the IEEE divide / sqrt costs throughput.
+#pragma once
+#include "hydro_math.cuh"
+
+namespace hyd {
+namespace fast {
+
+// 1/x, x > 0 finite and normal.  Seed has ~20 good bits; two Newton steps (measured on B200:
+// equal to the IEEE quotient on 2^26 arguments; one step leaves 4e3 ulp).
+__device__ __forceinline__ double rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    return y;
+}
+
+// 1/sqrt(x), x > 0 finite and normal.  One third-order step on the ~2^-20 seed: measured on
+// B200 |x y^2 - 1| <= 1.3 eps over 2^26 arguments (a second step does not improve on that).
+__device__ __forceinline__ double rsqrt(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y * y, 1.0);           // 1 - x y^2
+    const double p = fma(0.375, e, 0.5);
+    return fma(y, p * e, y);                        // y (1 + e/2 + 3 e^2/8)
+}
+
+// min of two non-negative doubles on the integer pipe (DSETP runs at half the DFMA rate on
+// sm_100a, measured; non-negative doubles order like their bit patterns)
+__device__ __forceinline__ double min_nonneg(double x, double y)
+{
+    return __double_as_longlong(x) < __double_as_longlong(y) ? x : y;
+}
+
+// O2: conserved -> primitive (rho, vx, vy, vz, p)
+__device__ __forceinline__ void prim5(const double U[5], double gm1, double W[5])
+{
+    const double inv = rcp(U[0]);
+    W[0] = U[0];
+    W[1] = U[1] * inv; W[2] = U[2] * inv; W[3] = U[3] * inv;
+    const double q = fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3]));
+    W[4] = gm1 * fma(-0.5 * U[0], q, U[4]);
+}
+
+// O3: limited slope of one cell; hs = 0.5 * sigma is formed directly:
+//   0.5*min(theta|a|, theta|b|, 0.5|a+b|) = min((0.5 theta) min(|a|,|b|), 0.25|a+b|)
+// (exactly, scaling by powers of two and monotone rounding), sign of a when a and b agree in
+// sign, else zero -- decided on the sign bits.
+__device__ __forceinline__ void limited_faces(double half_theta, const double Wm[5],
+                                              const double Wc[5], const double Wp[5],
+                                              double inner[5], double outer[5])
+{
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        const double a = Wc[v] - Wm[v];
+        const double b = Wp[v] - Wc[v];
+        const double mn = fabs(a) < fabs(b) ? a : b;
+        const double t1 = half_theta * fabs(mn);
+        const double t2 = 0.25 * fabs(a + b);
+        const double h = min_nonneg(t1, t2);
+        const int ah = __double2hiint(a), bh = __double2hiint(b);
+        const bool same = (ah ^ bh) >= 0;
+        const int hh = __double2hiint(h) | (ah & 0x80000000);
+        const double hs = __hiloint2double(same ? hh : 0, same ? __double2loint(h) : 0);
+        inner[v] = Wc[v] - hs;
+        outer[v] = Wc[v] + hs;
+    }
+}
+
+// O4: HLL flux, components in (rho, n, t1, t2, E) order; inputs (rho, vn, vt1, vt2, p).
+__device__ __forceinline__ void hll_flux(const double L[5], const double R[5], double gamma,
+                                         double igm1, double F[5])
+{
+    double UL[5], UR[5], FL[5], FR[5], cL, cR;
+    {
+        const double gp = gamma * L[4];
+        cL = gp * rsqrt(gp * L[0]);
+        const double k = fma(L[1], L[1], fma(L[2], L[2], L[3] * L[3]));
+        const double E = fma(0.5 * L[0], k, L[4] * igm1);
+        UL[0] = L[0]; UL[1] = L[0] * L[1]; UL[2] = L[0] * L[2]; UL[3] = L[0] * L[3]; UL[4] = E;
+        FL[0] = UL[1]; FL[1] = fma(UL[1], L[1], L[4]); FL[2] = UL[2] * L[1]; FL[3] = UL[3] * L[1];
+        FL[4] = (E + L[4]) * L[1];
+    }
+    {
+        const double gp = gamma * R[4];
+        cR = gp * rsqrt(gp * R[0]);
+        const double k = fma(R[1], R[1], fma(R[2], R[2], R[3] * R[3]));
+        const double E = fma(0.5 * R[0], k, R[4] * igm1);
+        UR[0] = R[0]; UR[1] = R[0] * R[1]; UR[2] = R[0] * R[2]; UR[3] = R[0] * R[3]; UR[4] = E;
+        FR[0] = UR[1]; FR[1] = fma(UR[1], R[1], R[4]); FR[2] = UR[2] * R[1]; FR[3] = UR[3] * R[1];
+        FR[4] = (E + R[4]) * R[1];
+    }
+    const double ap = dmax(0.0, dmax(L[1] + cL, R[1] + cR));
+    const double am = dmax(0.0, dmax(cL - L[1], cR - R[1]));
+    const double w = rcp(ap + am);
+    const double al = ap * w, be = am * w, de = (ap * am) * w;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        const double f = fma(al, FL[v], be * FR[v]);
+        F[v] = __fma_rn(-de, UR[v] - UL[v], f);
+    }
+}
+
+}  // namespace fast
+}  // namespace hyd

@@ -1,22 +1,109 @@
-// hydro_stage_fused.cuh -- placeholder until the tiled fused stage kernel lands (next commit).
+// hydro_stage_fused.cuh -- the fused RK-stage kernel (A2-A8 of DESIGN.md section 2) for sm_100a.
+//
+// One launch per Runge-Kutta substep does primitive recovery, the three per-dimension limited
+// reconstructions, the HLL face fluxes, the flux divergence, the stage combination and (stage 2)
+// the max-signal-speed reduction, i.e. the paper's ComputeDifferences / ComputeReconstruction /
+// ComputeFluxes / ComputeUpdate and the "FluidCurrent = ..." lines of Algorithm 1
+// without any of its intermediate storages.
+//
+// Shape.  The kernel is bound by the fp64 pipe, not by HBM, so the design
+// minimises fp64 instructions per cell: every slope and every face flux is computed exactly once.
+//   * A block owns a TX x TY column tile (x fastest, one warp per x-row of 32 cells) and marches
+//     along z over a chunk of `lz` planes.  A thread owns the column (i, j).
+//   * z direction: a register pipeline.  When plane kk arrives the thread has W(kk-2), W(kk-1),
+//     computes W(kk), the z-slope of cell kk-1 and the flux through face (kk-2)+1/2, which
+//     completes cell kk-2.  Nothing in z is ever recomputed or exchanged.
+//   * x and y directions of plane kk-2: primitives of (tile + 2-cell plus-shaped halo) go to
+//     shared memory once; each thread computes the slopes of its own cell, hands its outer face
+//     value to the +x / +y neighbour through shared memory, computes the flux through its low
+//     face and hands that to the -x / -y neighbour's divergence.  The tile's extra high-edge
+//     faces and the two halo-cell slopes they need are a flattened list done by the first warps.
+//   * conserved state crosses HBM once per stage (interior planes; halos and the two warm-up
+//     planes per chunk re-read through L2).
 #pragma once
 #include "hydro_kernels.cuh"
+#ifndef HYDRO_VERIFY
+#include "hydro_math_fast.cuh"
+#endif
 
 namespace hyd {
 
-struct FusedPlan { int ready = 0; };
+constexpr int FTX = 32;            // tile width: one warp per row
 
-inline cudaError_t plan_stage_fused(FusedPlan &, const Grid &, const double *, const double *)
+template <int TY> struct FusedSmem {
+    static constexpr int WP = FTX + 4;                 // pitch of the primitive tile
+    static constexpr int WROWS = TY + 4;
+    static constexpr int WSZ = WROWS * WP;             // per variable
+    static constexpr int XP = FTX + 2;                 // pitch of x-face arrays (FTX+1 used)
+    static constexpr int XSZ = TY * XP;
+    static constexpr int YSZ = (TY + 1) * FTX;
+    static constexpr int OFF_W = 0;
+    static constexpr int OFF_OX = OFF_W + NVAR * WSZ;  // outer x-face value of cell i-1 at slot i
+    static constexpr int OFF_OY = OFF_OX + NVAR * XSZ; // outer y-face value of row j-1 at row j
+    static constexpr int OFF_FX = OFF_OY + NVAR * YSZ; // flux through face i-1/2 at slot i
+    static constexpr int OFF_FY = OFF_FX + NVAR * XSZ;
+    static constexpr int OFF_IXE = OFF_FY + NVAR * YSZ; // inner x-face value of cell i0+TX, per row
+    static constexpr int OFF_IYE = OFF_IXE + NVAR * TY; // inner y-face value of row j0+TY, per col
+    static constexpr int TOTAL = OFF_IYE + NVAR * FTX;
+    static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
+};
+
+// ---- per-direction helpers: primitives are always held as (rho, vx, vy, vz, p) -----------------
+
+// slope of one cell from its two neighbours along a direction; returns inner and outer values
+__device__ __forceinline__ void limited_faces(double theta, const double Wm[5], const double Wc[5],
+                                              const double Wp[5], double inner[5], double outer[5])
 {
-    return cudaSuccess;
+#pragma unroll
+    for (int v = 0; v < 5; ++v) {
+        const double a = Wc[v] - Wm[v];
+        const double b = Wp[v] - Wc[v];
+        const double s = minmod(theta, a, b);
+        inner[v] = Wc[v] - 0.5 * s;
+        outer[v] = Wc[v] + 0.5 * s;
+    }
+}
+#ifndef HYDRO_VERIFY
+#define HYD_LIMITED_FACES(theta, Wm, Wc, Wp, In, Ou) fast::limited_faces(0.5 * (theta), Wm, Wc, Wp, In, Ou)
+#define HYD_HLL fast::hll_flux
+#define HYD_PRIM5 fast::prim5
+#define HYD_SUM3(x, y, z) (((x) + (y)) + (z))
+#else
+#define HYD_LIMITED_FACES(theta, Wm, Wc, Wp, In, Ou) limited_faces(theta, Wm, Wc, Wp, In, Ou)
+#define HYD_HLL hll_flux
+#define HYD_PRIM5 prim5
+#define HYD_SUM3(x, y, z) sum3(x, y, z)
+#endif
+
+// HLL flux through a face with normal D; L, R in (rho,vx,vy,vz,p); F in (rho,mx,my,mz,E) order
+template <int D>
+__device__ __forceinline__ void face_flux(const double L[5], const double R[5], double gamma,
+                                          double igm1, double F[5])
+{
+    const double l[5] = { L[0], L[1 + D], L[1 + (D + 1) % 3], L[1 + (D + 2) % 3], L[4] };
+    const double r[5] = { R[0], R[1 + D], R[1 + (D + 1) % 3], R[1 + (D + 2) % 3], R[4] };
+    double f[5];
+    HYD_HLL(l, r, gamma, igm1, f);
+    F[0] = f[0];
+    F[1 + D] = f[1];
+    F[1 + (D + 1) % 3] = f[2];
+    F[1 + (D + 2) % 3] = f[3];
+    F[4] = f[4];
 }
 
-template <int STAGE>
-inline cudaError_t launch_stage_fused(const FusedPlan &, const Grid &, const double *, const double *,
-                                      double *, double, const StepScalars *, double, StepScalars *,
-                                      cudaStream_t)
+__device__ __forceinline__ void prim5(const double U[5], double gm1, double W[5])
 {
-    return cudaErrorNotSupported;
+    const Prim w = primitive(U[0], U[1], U[2], U[3], U[4], gm1);
+    W[0] = w.rho; W[1] = w.vx; W[2] = w.vy; W[3] = w.vz; W[4] = w.p;
+}
+
+__device__ __forceinline__ void load5(const double *__restrict__ U, long long sv, long long c,
+                                      double u[5])
+{
+#pragma unroll
+    for (int v = 0; v < 5; ++v) u[v] = __ldg(U + v * sv + c);
 }
 
 }  // namespace hyd
+
+#include "hydro_stage_fused_kernel.cuh"

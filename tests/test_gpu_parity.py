@@ -256,15 +256,21 @@ def test_config2_sphere128_hundred_steps():
     g, c, _, _ = _run_pair(cfg, U, False, None)
     a = g.get_state()
     assert_production_bar(a, c.get_state())
-    _assert_cubic_symmetry(a)
+    _assert_cubic_symmetry(a, exact=False)
 
 
-def _assert_cubic_symmetry(a):
+def _assert_cubic_symmetry(a, exact):
+    """P4.  Verification build: bitwise (it reproduces the oracle's symmetric association, R17).
+    Production build: FMA contraction and the plain three-term sum are not permutation-symmetric
+    in the last bit (R20), so the images must agree to roundoff, 1e-12 of the scale."""
     import itertools
+    s = scales(a)[:, None, None, None]
     for perm in itertools.permutations((0, 1, 2)):
-        assert np.array_equal(inputs.permute_axes(a, perm), a), perm
+        b = inputs.permute_axes(a, perm)
+        assert np.array_equal(b, a) if exact else (np.abs(b - a) <= 1e-12 * s).all(), perm
     for ax in range(3):
-        assert np.array_equal(inputs.reflect_axis(a, ax), a), ax
+        b = inputs.reflect_axis(a, ax)
+        assert np.array_equal(b, a) if exact else (np.abs(b - a) <= 1e-12 * s).all(), ax
 
 
 def test_config4_shape_noise_periodic_conservation_and_parity():
@@ -293,8 +299,16 @@ def test_config3_full_size_sampled_and_symmetry():
     g.run_steps(cfg.steps - 4)
     a = g.get_state()
     assert g.get_time()[1] == cfg.steps
-    _assert_cubic_symmetry(a)
+    _assert_cubic_symmetry(a, exact=False)
     assert a[0].min() == 0.125 and np.isfinite(a).all()
+    g.close()
+    # verification build at full size: 4 steps bit-identical to the oracle, then 20 more steps
+    # must keep the cubic symmetry bitwise (a property that holds at any size)
+    g, c, _, _ = _run_pair(cfg, U, True, None, steps=4)
+    assert np.array_equal(g.get_state(), c.get_state())
+    del c
+    g.run_steps(20)
+    _assert_cubic_symmetry(g.get_state(), exact=True)
 
 
 @pytest.mark.skipif(os.environ.get("HYDRO_FULL_PARITY") != "1",
