@@ -22,6 +22,7 @@
 //     planes per chunk re-read through L2).
 #pragma once
 #include "hydro_kernels.cuh"
+#include "hydro_tma.cuh"
 #ifndef HYDRO_VERIFY
 #include "hydro_math_fast.cuh"
 #endif
@@ -30,22 +31,31 @@ namespace hyd {
 
 constexpr int FTX = 32;            // tile width: one warp per row
 
+constexpr int FNS = 4;             // TMA ring depth: planes kk-2, kk-1, kk resident + kk+1 in flight
+
+// Shared-memory carve-up (doubles).  The ring stages and the primitive tile share one layout,
+// [v][row][col] with pitch WP -- the layout the TMA box arrives in.
 template <int TY> struct FusedSmem {
-    static constexpr int WP = FTX + 4;                 // pitch of the primitive tile
+    static constexpr int WP = FTX + 4;                 // pitch of a (tile + halo) plane
     static constexpr int WROWS = TY + 4;
     static constexpr int WSZ = WROWS * WP;             // per variable
+    static constexpr int STAGE = NVAR * WSZ;           // one ring stage (multiple of 16 doubles)
     static constexpr int XP = FTX + 2;                 // pitch of x-face arrays (FTX+1 used)
     static constexpr int XSZ = TY * XP;
     static constexpr int YSZ = (TY + 1) * FTX;
-    static constexpr int OFF_W = 0;
-    static constexpr int OFF_OX = OFF_W + NVAR * WSZ;  // outer x-face value of cell i-1 at slot i
-    static constexpr int OFF_OY = OFF_OX + NVAR * XSZ; // outer y-face value of row j-1 at row j
-    static constexpr int OFF_FX = OFF_OY + NVAR * YSZ; // flux through face i-1/2 at slot i
-    static constexpr int OFF_FY = OFF_FX + NVAR * XSZ;
-    static constexpr int OFF_IXE = OFF_FY + NVAR * YSZ; // inner x-face value of cell i0+TX, per row
+    static constexpr int OFF_RING = 0;                 // raw conserved planes, filled by TMA
+    static constexpr int OFF_W = OFF_RING + FNS * STAGE;  // primitives of the plane being updated
+    static constexpr int OFF_OX = OFF_W + STAGE;       // outer x-face value of cell i-1 at slot i;
+    static constexpr int OFF_FX = OFF_OX;              //   overwritten in place by the flux through i-1/2
+    static constexpr int OFF_OY = OFF_OX + NVAR * XSZ; // outer y-face value of row j-1 at row j;
+    static constexpr int OFF_FY = OFF_OY;              //   overwritten in place by the flux through j-1/2
+    static constexpr int OFF_IXE = OFF_OY + NVAR * YSZ; // inner x-face value of cell i0+TX, per row
     static constexpr int OFF_IYE = OFF_IXE + NVAR * TY; // inner y-face value of row j0+TY, per col
-    static constexpr int TOTAL = OFF_IYE + NVAR * FTX;
+    static constexpr int OFF_BAR = OFF_IYE + NVAR * FTX; // FNS mbarriers
+    static constexpr int TOTAL = OFF_BAR + FNS;
     static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
+    static constexpr unsigned STAGE_BYTES = STAGE * sizeof(double);
+    static_assert(STAGE_BYTES % 128 == 0, "TMA destination stages must stay 128-byte aligned");
 };
 
 // ---- per-direction helpers: primitives are always held as (rho, vx, vy, vz, p) -----------------
@@ -95,13 +105,6 @@ __device__ __forceinline__ void prim5(const double U[5], double gm1, double W[5]
 {
     const Prim w = primitive(U[0], U[1], U[2], U[3], U[4], gm1);
     W[0] = w.rho; W[1] = w.vx; W[2] = w.vy; W[3] = w.vz; W[4] = w.p;
-}
-
-__device__ __forceinline__ void load5(const double *__restrict__ U, long long sv, long long c,
-                                      double u[5])
-{
-#pragma unroll
-    for (int v = 0; v < 5; ++v) u[v] = __ldg(U + v * sv + c);
 }
 
 }  // namespace hyd
