@@ -47,6 +47,11 @@ __device__ __forceinline__ double min_nonneg(double x, double y)
     return __double_as_longlong(x) < __double_as_longlong(y) ? x : y;
 }
 
+__device__ __forceinline__ double max_nonneg(double x, double y)
+{
+    return __double_as_longlong(x) > __double_as_longlong(y) ? x : y;
+}
+
 // O2: conserved -> primitive (rho, vx, vy, vz, p)
 __device__ __forceinline__ void prim5(const double U[5], double gm1, double W[5])
 {
@@ -114,6 +119,24 @@ __device__ __forceinline__ void hll_flux(const double L[5], const double R[5], d
         const double f = fma(al, FL[v], be * FR[v]);
         F[v] = __fma_rn(-de, UR[v] - UL[v], f);
     }
+}
+
+// O7: signal speed |v| + c_s of one updated cell for the fused CFL reduction.  sqrt(x) is formed as
+// x * rsqrt(x + tiny) so that x = 0 gives 0 instead of NaN.  `bad` is raised on the sign/zero bits
+// of rho and p (integer pipe); a non-finite speed is caught once per thread from the running
+// maximum, whose bit pattern then compares above every finite value.
+__device__ __forceinline__ double signal_speed(const double U[5], double gamma, double gm1, int &bad)
+{
+    double W[5];
+    const double inv = rcp(U[0]);
+    W[1] = U[1] * inv; W[2] = U[2] * inv; W[3] = U[3] * inv;
+    const double q = fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3]));
+    const double p = gm1 * fma(-0.5 * U[0], q, U[4]);
+    const double c2 = (gamma * p) * inv;
+    const double tiny = 1e-300;
+    const double s = fma(q, rsqrt(q + tiny), c2 * rsqrt(c2 + tiny));
+    bad |= (__double_as_longlong(U[0]) <= 0ll) | (__double_as_longlong(p) <= 0ll);
+    return s;
 }
 
 }  // namespace fast

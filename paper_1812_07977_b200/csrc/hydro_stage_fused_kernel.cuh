@@ -239,12 +239,19 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg] = un[v];
             if (STAGE == 2 && a.red) {
+#ifdef HYDRO_VERIFY
                 const double s = cell_signal_speed(un[0], un[1], un[2], un[3], un[4], gamma, gm1, bad);
                 smax = s > smax ? s : smax;
+#else
+                smax = fast::max_nonneg(smax, fast::signal_speed(un, gamma, gm1, bad));
+#endif
             }
         }
     }
-    if (STAGE == 2 && a.red) block_max_to_global(smax, bad, &a.red->smax_bits, &a.red->flag);
+    if (STAGE == 2 && a.red) {
+        if (!(smax <= 1.79769313486231570e308)) { bad = 1; smax = 0.0; }   // inf or NaN pattern won
+        block_max_to_global(smax, bad, &a.red->smax_bits, &a.red->flag);
+    }
 }
 
 }  // namespace hyd
