@@ -16,6 +16,13 @@ struct FusedArgs {
 };
 
 // `umap` describes the stencil input (stage 1: U0, stage 2: U1; ghost-filled) to the TMA unit.
+//
+// Synchronisation.  The x/y exchange of one plane needs three block-wide hand-offs (primitives,
+// outer face values, fluxes).  Each is a split-phase mbarrier: a warp ARRIVES as soon as its
+// stores are done, then does z-direction work that needs no one else (the filler), and only then
+// WAITS.  The skew between warps is absorbed by the fillers instead of idling at a barrier.
+//   per cell plane c:  [prim(c+4), z-slope] wait_W  P2  arrive_O  [z-flux]  wait_O  P3  arrive_F
+//                      [primitive tile of plane c+1] arrive_W(c+1)  wait_F  P4
 template <int STAGE, int TY, int MINB>
 __global__ void __launch_bounds__(FTX * TY, MINB)
 stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
@@ -26,14 +33,16 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     double *Wsm = sm + S::OFF_W, *Oxs = sm + S::OFF_OX, *Oys = sm + S::OFF_OY;
     double *Fxs = sm + S::OFF_FX, *Fys = sm + S::OFF_FY;
     double *Ixe = sm + S::OFF_IXE, *Iye = sm + S::OFF_IYE;
-    uint64_t *bar = reinterpret_cast<uint64_t *>(sm + S::OFF_BAR);
+    uint64_t *bar = reinterpret_cast<uint64_t *>(sm + S::OFF_BAR);     // TMA: plane p -> bar[p % FNS]
+    uint64_t *barW = bar + FNS, *barO = bar + FNS + 1, *barF = bar + FNS + 2;
 
     const Grid &g = a.g;
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;     // tile origin, active coordinates
     const int k0 = blockIdx.z * a.lz;
     const int k1 = min(k0 + a.lz, g.nz);                      // chunk = active planes [k0, k1)
-    const int nplanes = k1 - k0 + 4;                          // planes k0-2 .. k1+1 stream through
+    const int nc = k1 - k0;                                   // cell planes; raw planes 0..nc+3
+    const int nplanes = nc + 4;                               //   (raw plane p = active plane k0-2+p)
     const double gamma = g.gamma, gm1 = g.gm1, igm1 = g.igm1, theta = g.theta;
     const long long sv = g.sv;
 
@@ -43,105 +52,111 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const long long col = (long long)(i0 + tx + NG) + (long long)g.px * (j0 + ty + NG);
     const int wc = (ty + 2) * WP + tx + 2;                    // own cell in a (tile + halo) plane
 
-    // halo cell of this thread (first 4*TY + 4*TX threads), plane coordinates (hc, hr)
+    // The tile's extra work (halo primitives, halo-cell slopes, high-edge faces) is a flattened
+    // list spread over the warps so that the four SM sub-partitions (warp % 4) carry equal loads:
+    // edge faces on warps 0,1; y halo slopes on warps 2,3; x halo slopes on warp 6; halo
+    // primitives on warps 3.. (x halo on warp 3, y halo on the following ones).
+    static_assert(TY >= 8, "role assignment needs at least 8 warps");
     constexpr int NHX = 4 * TY, NH = 4 * TY + 4 * TX;
+    const int th = t - 3 * TX;                                // halo cell index, plane coords (hc, hr)
     int hc = 0, hr = 0;
-    if (t < NHX) { const int q = t & 3; hr = (t >> 2) + 2; hc = q < 2 ? q : TX + q; }
-    else if (t < NH) { const int u = t - NHX, q = u / TX; hc = (u % TX) + 2; hr = q < 2 ? q : TY + q; }
-    const bool has_halo = t < NH;
-    const int hw = hr * WP + hc;
+    if (th < NHX) { const int q = th & 3; hr = (th >> 2) + 2; hc = q < 2 ? q : TX + q; }
+    else if (th < NH) { const int u = th - NHX, q = u / TX; hc = (u % TX) + 2; hr = q < 2 ? q : TY + q; }
+    const bool has_halo = th >= 0 && th < NH;
+    const int hw = has_halo ? hr * WP + hc : 0;
 
-    // ---- TMA ring: plane index p (0 = active plane k0-2) lives in stage p % FNS ----------------
     if (t == 0) {
 #pragma unroll
         for (int s = 0; s < FNS; ++s) tma::mbar_init(&bar[s], 1);
+        tma::mbar_init(barW, TY); tma::mbar_init(barO, TY); tma::mbar_init(barF, TY);
         tma::fence_barrier_init();
     }
     __syncthreads();
-    if (t == 0) {
-        const int np = nplanes < FNS ? nplanes : FNS;
-        for (int p = 0; p < np; ++p) {
-            tma::mbar_arrive_expect_tx(&bar[p], S::STAGE_BYTES);
-            tma::load_4d(sm + S::OFF_RING + p * S::STAGE, &umap, i0, j0, k0 + p, 0, &bar[p]);
-        }
-    }
+    auto request_plane = [&](int p) {                         // thread 0 only
+        tma::mbar_arrive_expect_tx(&bar[p % FNS], S::STAGE_BYTES);
+        tma::load_4d(sm + S::OFF_RING + (p % FNS) * S::STAGE, &umap, i0, j0, k0 + p, 0, &bar[p % FNS]);
+    };
+    if (t == 0)
+        for (int p = 0; p < FNS; ++p) request_plane(p);       // nplanes >= 5 > FNS
 
     const double r = a.dev_dt ? a.dev_dt->dt / a.dx : a.dt_over_dx;
 
-    double Wa[5], Wb[5];          // W(kk-2), W(kk-1)
-    double Oz[5];                 // outer z-face value of cell kk-2
-    double Fzm[5];                // flux through face (kk-2)-1/2
+    // primitive tile of one cell plane: own cell from registers, halo cells from the raw plane
+    auto write_tile = [&](const double Wown[5], const double *Uraw) {
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + wc] = Wown[v];
+        if (has_halo) {
+            double Uh[5], Wh[5];
+#pragma unroll
+            for (int v = 0; v < 5; ++v) Uh[v] = Uraw[v * S::WSZ + hw];
+            HYD_PRIM5(Uh, gm1, Wh);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + hw] = Wh[v];
+        }
+        __syncwarp();
+        if (tx == 0) tma::mbar_arrive(barW);
+    };
+
+    // ---- prologue: raw planes 0..3 -> W(k0), W(k0+1), outer_z(k0), flux through face k0-1/2 ----
+    double Wa[5], Wb[5];          // W(k), W(k+1) of the current cell plane k
+    double Oz[5];                 // outer z-face value of cell k
+    double Fzm[5];                // flux through face k-1/2
     double smax = 0.0;
     int bad = 0;
 #pragma unroll
     for (int v = 0; v < 5; ++v) { Wa[v] = Wb[v] = Oz[v] = Fzm[v] = 0.0; }
-
 #pragma unroll 1
-    for (int p = 0; p < nplanes; ++p) {
-        const int kk = k0 - 2 + p;
-        const bool do_slope = p >= 2, do_flux = p >= 3, do_cell = p >= 4;
-        const double *Ucur = sm + S::OFF_RING + (p % FNS) * S::STAGE;          // raw plane kk
-        const double *Uk = sm + S::OFF_RING + ((p + 2) % FNS) * S::STAGE;      // raw plane kk-2
-        tma::mbar_wait(&bar[p % FNS], (p / FNS) & 1);
-        // ---------------- phase 1: primitives of the new plane; z pipeline -------------------
-        double Wn[5];
-        {
-            double Un[5];
+    for (int p = 0; p < 4; ++p) {
+        tma::mbar_wait(&bar[p], 0);
+        double Un[5], Wn[5];
 #pragma unroll
-            for (int v = 0; v < 5; ++v) Un[v] = Ucur[v * S::WSZ + wc];
-            HYD_PRIM5(Un, gm1, Wn);
-        }
-        double dFz[5];
-        if (do_slope) {
+        for (int v = 0; v < 5; ++v) Un[v] = sm[S::OFF_RING + p * S::STAGE + v * S::WSZ + wc];
+        HYD_PRIM5(Un, gm1, Wn);
+        if (p >= 2) {
             double Iz[5], Ozn[5];
-            HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);    // cell kk-1
-            if (do_flux) {
-                double Fzp[5];
-                face_flux<2>(Oz, Iz, gamma, igm1, Fzp);       // face (kk-2)+1/2
-#pragma unroll
-                for (int v = 0; v < 5; ++v) { dFz[v] = Fzp[v] - Fzm[v]; Fzm[v] = Fzp[v]; }
-            }
+            HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);    // cell of raw plane p-1
+            if (p == 3) face_flux<2>(Oz, Iz, gamma, igm1, Fzm);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Oz[v] = Ozn[v];
         }
-        double Wc[5];
 #pragma unroll
-        for (int v = 0; v < 5; ++v) { Wc[v] = Wa[v]; Wa[v] = Wb[v]; Wb[v] = Wn[v]; }
-        if (do_cell) {
-#pragma unroll
-            for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + wc] = Wc[v];
-            if (has_halo) {
-                double Uh[5], Wh[5];
-#pragma unroll
-                for (int v = 0; v < 5; ++v) Uh[v] = Uk[v * S::WSZ + hw];
-                HYD_PRIM5(Uh, gm1, Wh);
-#pragma unroll
-                for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + hw] = Wh[v];
-            }
+        for (int v = 0; v < 5; ++v) { Wa[v] = Wb[v]; Wb[v] = Wn[v]; }
+        if (p == 1) {                                         // raw plane 0 has been read by everyone
+            __syncthreads();
+            if (t == 0) { tma::fence_proxy_async(); request_plane(4); }
         }
-        __syncthreads();
-        // every thread is past its reads of plane p-3 (stage (p+1) % FNS): refill it with p+1
-        if (t == 0 && p + 1 >= FNS && p + 1 < nplanes) {
-            tma::fence_proxy_async();
-            tma::mbar_arrive_expect_tx(&bar[(p + 1) % FNS], S::STAGE_BYTES);
-            tma::load_4d(sm + S::OFF_RING + ((p + 1) % FNS) * S::STAGE, &umap, i0, j0, k0 + p + 1, 0,
-                         &bar[(p + 1) % FNS]);
+    }
+    write_tile(Wa, sm + S::OFF_RING + 2 * S::STAGE);          // cell plane 0 = raw plane 2; arrive_W(0)
+
+#pragma unroll 1
+    for (int c = 0; c < nc; ++c) {
+        const uint32_t par = c & 1;
+        const double *Uk = sm + S::OFF_RING + ((c + 2) % FNS) * S::STAGE;      // raw plane of cell plane c
+        const long long cg = col + g.sy * (long long)(k0 + c + NG);
+        // ---- filler W: primitives of raw plane c+4, z-slope of cell plane c+1 ---------------
+        double Wn[5], Iz[5], Ozn[5];
+        {
+            const int p = c + 4;
+            tma::mbar_wait(&bar[p % FNS], (p / FNS) & 1);
+            double Un[5];
+#pragma unroll
+            for (int v = 0; v < 5; ++v) Un[v] = sm[S::OFF_RING + (p % FNS) * S::STAGE + v * S::WSZ + wc];
+            HYD_PRIM5(Un, gm1, Wn);
+            HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
-        if (!do_cell) continue;
-        const int k = kk - 2;                                 // the plane completed this iteration
-        const long long cg = col + g.sy * (long long)(k + NG);
         if (STAGE == 2 && active) {
 #pragma unroll
             for (int v = 0; v < 5; ++v)
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Uold + v * sv + cg));
         }
-        // ---------------- phase 2: x and y slopes, face values -------------------------------
+        tma::mbar_wait(barW, par);
+        // ---- P2: x and y slopes of the own cell (W(k) = Wa), outer face values out ----------
         double Ix[5], Iy[5];
         {
             double Wm[5], Wp[5], Ox[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { Wm[v] = Wsm[v * S::WSZ + wc - 1]; Wp[v] = Wsm[v * S::WSZ + wc + 1]; }
-            HYD_LIMITED_FACES(theta, Wm, Wc, Wp, Ix, Ox);
+            HYD_LIMITED_FACES(theta, Wm, Wa, Wp, Ix, Ox);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Oxs[v * S::XSZ + ty * XP + tx + 1] = Ox[v];
         }
@@ -149,36 +164,50 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             double Wm[5], Wp[5], Oy[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { Wm[v] = Wsm[v * S::WSZ + wc - WP]; Wp[v] = Wsm[v * S::WSZ + wc + WP]; }
-            HYD_LIMITED_FACES(theta, Wm, Wc, Wp, Iy, Oy);
+            HYD_LIMITED_FACES(theta, Wm, Wa, Wp, Iy, Oy);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Oys[v * S::YSZ + (ty + 1) * TX + tx] = Oy[v];
         }
         // halo-cell slopes: x: cells (-1, j) -> outer, (TX, j) -> inner; y: rows -1 -> outer, TY -> inner
-        if (t < 2 * TY + 2 * TX) {
-            int c, st, dst, dstride;
+        if (ty == 2 || ty == 3 || (ty == 6 && tx < 2 * TY)) {
+            int cc, st, dst, dstride;
             bool want_outer;
-            if (t < 2 * TY) {
-                const int j = t >> 1, hi = t & 1;
-                c = (j + 2) * WP + (hi ? TX + 2 : 1); st = 1; want_outer = !hi;
+            if (ty == 6) {
+                const int j = tx >> 1, hi = tx & 1;
+                cc = (j + 2) * WP + (hi ? TX + 2 : 1); st = 1; want_outer = !hi;
                 dst = hi ? S::OFF_IXE + j : S::OFF_OX + j * XP;
                 dstride = hi ? TY : S::XSZ;
             } else {
-                const int u = t - 2 * TY, hi = u / TX, i = u % TX;
-                c = (hi ? TY + 2 : 1) * WP + i + 2; st = WP; want_outer = !hi;
+                const int hi = ty - 2, i = tx;
+                cc = (hi ? TY + 2 : 1) * WP + i + 2; st = WP; want_outer = !hi;
                 dst = hi ? S::OFF_IYE + i : S::OFF_OY + i;
                 dstride = hi ? TX : S::YSZ;
             }
             double Wm[5], W0[5], Wp[5], In[5], Ou[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) {
-                Wm[v] = Wsm[v * S::WSZ + c - st]; W0[v] = Wsm[v * S::WSZ + c]; Wp[v] = Wsm[v * S::WSZ + c + st];
+                Wm[v] = Wsm[v * S::WSZ + cc - st]; W0[v] = Wsm[v * S::WSZ + cc]; Wp[v] = Wsm[v * S::WSZ + cc + st];
             }
             HYD_LIMITED_FACES(theta, Wm, W0, Wp, In, Ou);
 #pragma unroll
             for (int v = 0; v < 5; ++v) sm[dst + v * dstride] = want_outer ? Ou[v] : In[v];
         }
-        __syncthreads();
-        // ---------------- phase 3: x and y fluxes through the low faces ----------------------
+        __syncwarp();
+        if (tx == 0) tma::mbar_arrive(barO);
+        // ---- filler O: z flux through face k+1/2; rotate the z pipeline ---------------------
+        double dFz[5];
+        {
+            double Fzp[5];
+            face_flux<2>(Oz, Iz, gamma, igm1, Fzp);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                dFz[v] = Fzp[v] - Fzm[v]; Fzm[v] = Fzp[v]; Oz[v] = Ozn[v]; Wa[v] = Wb[v]; Wb[v] = Wn[v];
+            }
+        }
+        tma::mbar_wait(barO, par);
+        // every warp is past P4 of cell plane c-1: raw plane c+1 is dead, refill its stage
+        if (t == 0 && c + 5 < nplanes) { tma::fence_proxy_async(); request_plane(c + 5); }
+        // ---- P3: x and y fluxes through the low faces ---------------------------------------
         double Fxl[5], Fyl[5];
         {
             double L[5];
@@ -213,13 +242,17 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) Fys[v * S::YSZ + TY * TX + tx] = F[v];
         }
+        __syncwarp();
+        if (tx == 0) tma::mbar_arrive(barF);
+        // ---- filler F: U0 loads in flight (stage 2); primitive tile of cell plane c+1 --------
         double Uo[5];
-        if (STAGE == 2) {                                     // in flight across the barrier
+        if (STAGE == 2) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) Uo[v] = active ? a.Uold[v * sv + cg] : 0.0;
         }
-        __syncthreads();
-        // ---------------- phase 4: divergence, RK combine, store, CFL ------------------------
+        if (c + 1 < nc) write_tile(Wa, sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE);   // arrive_W(c+1)
+        tma::mbar_wait(barF, par);
+        // ---- P4: divergence, RK combine, store, CFL ------------------------------------------
         double un[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
