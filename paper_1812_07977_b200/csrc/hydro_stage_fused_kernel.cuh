@@ -21,8 +21,8 @@ struct FusedArgs {
 // outer face values, fluxes).  Each is a split-phase mbarrier: a warp ARRIVES as soon as its
 // stores are done, then does z-direction work that needs no one else (the filler), and only then
 // WAITS.  The skew between warps is absorbed by the fillers instead of idling at a barrier.
-//   per cell plane c:  [prim(c+4), z-slope] wait_W  P2  arrive_O  [z-flux]  wait_O  P3  arrive_F
-//                      [primitive tile of plane c+1] arrive_W(c+1)  wait_F  P4
+//   per cell plane c:  wait_W  P2  arrive_O  [prim(c+4), z-slope]  wait_O  P3  arrive_F
+//                      [z-flux, primitive tile of plane c+1, arrive_W(c+1)]  wait_F  P4
 template <int STAGE, int TY, int MINB>
 __global__ void __launch_bounds__(FTX * TY, MINB)
 stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
@@ -53,17 +53,13 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const int wc = (ty + 2) * WP + tx + 2;                    // own cell in a (tile + halo) plane
 
     // The tile's extra work (halo primitives, halo-cell slopes, high-edge faces) is a flattened
-    // list spread over the warps so that the four SM sub-partitions (warp % 4) carry equal loads:
-    // edge faces on warps 0,1; y halo slopes on warps 2,3; x halo slopes on warp 6; halo
-    // primitives on warps 3.. (x halo on warp 3, y halo on the following ones).
-    static_assert(TY >= 8, "role assignment needs at least 8 warps");
+    // list handed out by ROLE = (warp + plane) mod TY, so that it rotates over the warps from plane
+    // to plane: every warp (and every SM sub-partition, warp % 4) carries the same load over TY
+    // planes, and the short-term imbalance stays inside the slack of the split barriers.
+    //   roles 0,1: high-edge x / y faces;  roles 2,3: y halo slopes;  role 6: x halo slopes;
+    //   roles 3..: halo primitives (x halo on role 3, y halo on the following ones).
+    static_assert(TY >= 8 && (TY & (TY - 1)) == 0, "role rotation needs a power-of-two warp count >= 8");
     constexpr int NHX = 4 * TY, NH = 4 * TY + 4 * TX;
-    const int th = t - 3 * TX;                                // halo cell index, plane coords (hc, hr)
-    int hc = 0, hr = 0;
-    if (th < NHX) { const int q = th & 3; hr = (th >> 2) + 2; hc = q < 2 ? q : TX + q; }
-    else if (th < NH) { const int u = th - NHX, q = u / TX; hc = (u % TX) + 2; hr = q < 2 ? q : TY + q; }
-    const bool has_halo = th >= 0 && th < NH;
-    const int hw = has_halo ? hr * WP + hc : 0;
 
     if (t == 0) {
 #pragma unroll
@@ -82,10 +78,15 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const double r = a.dev_dt ? a.dev_dt->dt / a.dx : a.dt_over_dx;
 
     // primitive tile of one cell plane: own cell from registers, halo cells from the raw plane
-    auto write_tile = [&](const double Wown[5], const double *Uraw) {
+    auto write_tile = [&](const double Wown[5], const double *Uraw, int role) {
 #pragma unroll
         for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + wc] = Wown[v];
-        if (has_halo) {
+        const int th = (role - 3) * TX + tx;                  // halo cell index -> plane coords (hc, hr)
+        if (th >= 0 && th < NH) {
+            int hc, hr;
+            if (th < NHX) { const int q = th & 3; hr = (th >> 2) + 2; hc = q < 2 ? q : TX + q; }
+            else { const int u = th - NHX, q = u / TX; hc = (u % TX) + 2; hr = q < 2 ? q : TY + q; }
+            const int hw = hr * WP + hc;
             double Uh[5], Wh[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) Uh[v] = Uraw[v * S::WSZ + hw];
@@ -126,24 +127,14 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             if (t == 0) { tma::fence_proxy_async(); request_plane(4); }
         }
     }
-    write_tile(Wa, sm + S::OFF_RING + 2 * S::STAGE);          // cell plane 0 = raw plane 2; arrive_W(0)
+    write_tile(Wa, sm + S::OFF_RING + 2 * S::STAGE, ty);      // cell plane 0 = raw plane 2; arrive_W(0)
 
 #pragma unroll 1
     for (int c = 0; c < nc; ++c) {
         const uint32_t par = c & 1;
+        const int role = (ty + c) & (TY - 1);
         const double *Uk = sm + S::OFF_RING + ((c + 2) % FNS) * S::STAGE;      // raw plane of cell plane c
         const long long cg = col + g.sy * (long long)(k0 + c + NG);
-        // ---- filler W: primitives of raw plane c+4, z-slope of cell plane c+1 ---------------
-        double Wn[5], Iz[5], Ozn[5];
-        {
-            const int p = c + 4;
-            tma::mbar_wait(&bar[p % FNS], (p / FNS) & 1);
-            double Un[5];
-#pragma unroll
-            for (int v = 0; v < 5; ++v) Un[v] = sm[S::OFF_RING + (p % FNS) * S::STAGE + v * S::WSZ + wc];
-            HYD_PRIM5(Un, gm1, Wn);
-            HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
-        }
         if (STAGE == 2 && active) {
 #pragma unroll
             for (int v = 0; v < 5; ++v)
@@ -169,16 +160,16 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             for (int v = 0; v < 5; ++v) Oys[v * S::YSZ + (ty + 1) * TX + tx] = Oy[v];
         }
         // halo-cell slopes: x: cells (-1, j) -> outer, (TX, j) -> inner; y: rows -1 -> outer, TY -> inner
-        if (ty == 2 || ty == 3 || (ty == 6 && tx < 2 * TY)) {
+        if (role == 2 || role == 3 || (role == 6 && tx < 2 * TY)) {
             int cc, st, dst, dstride;
             bool want_outer;
-            if (ty == 6) {
+            if (role == 6) {
                 const int j = tx >> 1, hi = tx & 1;
                 cc = (j + 2) * WP + (hi ? TX + 2 : 1); st = 1; want_outer = !hi;
                 dst = hi ? S::OFF_IXE + j : S::OFF_OX + j * XP;
                 dstride = hi ? TY : S::XSZ;
             } else {
-                const int hi = ty - 2, i = tx;
+                const int hi = role - 2, i = tx;
                 cc = (hi ? TY + 2 : 1) * WP + i + 2; st = WP; want_outer = !hi;
                 dst = hi ? S::OFF_IYE + i : S::OFF_OY + i;
                 dstride = hi ? TX : S::YSZ;
@@ -194,15 +185,16 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         }
         __syncwarp();
         if (tx == 0) tma::mbar_arrive(barO);
-        // ---- filler O: z flux through face k+1/2; rotate the z pipeline ---------------------
-        double dFz[5];
+        // ---- filler O: primitives of raw plane c+4, z-slope of cell plane c+1 ---------------
+        double Wn[5], Iz[5], Ozn[5];
         {
-            double Fzp[5];
-            face_flux<2>(Oz, Iz, gamma, igm1, Fzp);
+            const int p = c + 4;
+            tma::mbar_wait(&bar[p % FNS], (p / FNS) & 1);
+            double Un[5];
 #pragma unroll
-            for (int v = 0; v < 5; ++v) {
-                dFz[v] = Fzp[v] - Fzm[v]; Fzm[v] = Fzp[v]; Oz[v] = Ozn[v]; Wa[v] = Wb[v]; Wb[v] = Wn[v];
-            }
+            for (int v = 0; v < 5; ++v) Un[v] = sm[S::OFF_RING + (p % FNS) * S::STAGE + v * S::WSZ + wc];
+            HYD_PRIM5(Un, gm1, Wn);
+            HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
         tma::mbar_wait(barO, par);
         // every warp is past P4 of cell plane c-1: raw plane c+1 is dead, refill its stage
@@ -225,16 +217,16 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) Fys[v * S::YSZ + ty * TX + tx] = Fyl[v];
         }
-        // the tile's high-edge faces: warp 0 lanes < TY: x face of row `lane`; warp 1: y face of
+        // the tile's high-edge faces: role 0 lanes < TY: x face of row `lane`; role 1: y face of
         // column `lane` (each flux is written over the outer value it consumed)
-        if (ty == 0 && tx < TY) {
+        if (role == 0 && tx < TY) {
             double L[5], R[5], F[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { L[v] = Oxs[v * S::XSZ + tx * XP + TX]; R[v] = Ixe[v * TY + tx]; }
             face_flux<0>(L, R, gamma, igm1, F);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Fxs[v * S::XSZ + tx * XP + TX] = F[v];
-        } else if (ty == 1) {
+        } else if (role == 1) {
             double L[5], R[5], F[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { L[v] = Oys[v * S::YSZ + TY * TX + tx]; R[v] = Iye[v * TX + tx]; }
@@ -244,13 +236,24 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         }
         __syncwarp();
         if (tx == 0) tma::mbar_arrive(barF);
-        // ---- filler F: U0 loads in flight (stage 2); primitive tile of cell plane c+1 --------
+        // ---- filler F: U0 loads in flight (stage 2) ------------------------------------------
         double Uo[5];
         if (STAGE == 2) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) Uo[v] = active ? a.Uold[v * sv + cg] : 0.0;
         }
-        if (c + 1 < nc) write_tile(Wa, sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE);   // arrive_W(c+1)
+        // z flux through face k+1/2; rotate the z pipeline; primitive tile of cell plane c+1
+        double dFz[5];
+        {
+            double Fzp[5];
+            face_flux<2>(Oz, Iz, gamma, igm1, Fzp);
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                dFz[v] = Fzp[v] - Fzm[v]; Fzm[v] = Fzp[v]; Oz[v] = Ozn[v]; Wa[v] = Wb[v]; Wb[v] = Wn[v];
+            }
+        }
+        if (c + 1 < nc)                                       // arrive_W(c+1)
+            write_tile(Wa, sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE, (ty + c + 1) & (TY - 1));
         tma::mbar_wait(barF, par);
         // ---- P4: divergence, RK combine, store, CFL ------------------------------------------
         double un[5];
