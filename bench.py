@@ -151,7 +151,7 @@ def time_oracle(cfg, steps, warmup, nzs):
     return cells * steps / el, el, oracle.get_threads(), cells
 
 
-def cpu_baseline(cfg, budget_s=15.0):
+def cpu_baseline(cfg, budget_s=20.0):
     """Oracle as it stands on the host cores, on a bounded sample (~10-30 s of CPU work)."""
     nz = cfg.shape[2]
     rate, _, cores, _ = time_oracle(cfg, 1, 0, min(nz, 32))      # calibrate (also warms up)
