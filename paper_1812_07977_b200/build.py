@@ -19,7 +19,7 @@ HEADERS = ["hydro_math.cuh", "hydro_math_fast.cuh", "hydro_kernels.cuh", "hydro_
 LIB = os.path.join(HERE, "libhydro_b200.so")
 LIB_VERIFY = os.path.join(HERE, "libhydro_b200_verify.so")
 
-COMMON = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
+COMMON = os.environ.get("HYD_EXTRA_NVCC", "").split() + ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
           "-Xcompiler", "-fPIC", "-shared", "-Xptxas", "-v"]
 
 

@@ -135,11 +135,6 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         const int role = (ty + c) & (TY - 1);
         const double *Uk = sm + S::OFF_RING + ((c + 2) % FNS) * S::STAGE;      // raw plane of cell plane c
         const long long cg = col + g.sy * (long long)(k0 + c + NG);
-        if (STAGE == 2 && active) {
-#pragma unroll
-            for (int v = 0; v < 5; ++v)
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Uold + v * sv + cg));
-        }
         tma::mbar_wait(barW, par);
         // ---- P2: x and y slopes of the own cell (W(k) = Wa), outer face values out ----------
         double Ix[5], Iy[5];
