@@ -64,6 +64,10 @@ struct hydro {
     long long step = 0;
     int variant = 1;
     FusedPlan plan;                 // launch geometry / TMA descriptors of the fused kernel
+    // one device-dt RK2 step (next_dt + stage launches) captured as a CUDA graph, replayed by
+    // hydro_run_steps / hydro_evolve; rebuilt when anything baked into the launches changes
+    cudaGraphExec_t step_graph = nullptr;
+    int graph_kernels = 0;          // kernels per replay (for hydro_launch_count)
     // measurement hooks (hydro_set_profiling)
     bool profiling = false;
     struct Span { int which; cudaEvent_t a, b; };
@@ -238,6 +242,63 @@ int copy_state(hydro *h, double *padded, double *packed, bool to_padded)
     return HYDRO_OK;
 }
 
+void drop_graph(hydro *h)
+{
+    if (h->step_graph) { cudaGraphExecDestroy(h->step_graph); h->step_graph = nullptr; }
+}
+
+int launch_next_dt(hydro *h)
+{
+    {
+        Scope sc(h, K_NEXTDT);
+        next_dt_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->cfl, h->dx);
+    }
+    LAUNCH_CHECK("next_dt");
+    return HYDRO_OK;
+}
+
+// n device-dt steps: replays of the captured one-step graph when possible (not on the legacy
+// default stream, which cannot be captured, and not while per-kernel profiling is on).
+int enqueue_device_steps(hydro *h, long long n)
+{
+    int rc;
+    const bool use_graph = h->stream != nullptr && !h->profiling && !getenv("HYDRO_NO_GRAPH");
+    if (use_graph && !h->step_graph) {
+        const long long before = g_launches.load();
+        cudaGraph_t graph = nullptr;
+        CUDA_TRY(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
+        rc = launch_next_dt(h);
+        if (!rc) rc = enqueue_step(h, 0.0, true);
+        cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
+        if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "graph capture: %s%s", cudaGetErrorString(e));
+        e = cudaGraphInstantiate(&h->step_graph, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) { h->step_graph = nullptr; return fail(HYDRO_ERR_CUDA, "graph instantiate: %s%s", cudaGetErrorString(e)); }
+        h->graph_kernels = (int)(g_launches.load() - before);
+        g_launches.store(before);                     // capture launched nothing
+    }
+    for (long long s = 0; s < n; ++s) {
+        if (use_graph) {
+            CUDA_TRY(cudaGraphLaunch(h->step_graph, h->stream));
+            g_launches.fetch_add(h->graph_kernels, std::memory_order_relaxed);
+        } else {
+            if ((rc = launch_next_dt(h))) return rc;
+            if ((rc = enqueue_step(h, 0.0, true))) return rc;
+        }
+    }
+    h->smax_valid = true;
+    return HYDRO_OK;
+}
+
+int begin_run(hydro *h, double t_final)
+{
+    begin_run_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->t, t_final);
+    LAUNCH_CHECK("begin_run");
+    h->t_on_device = true;
+    return HYDRO_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -349,6 +410,7 @@ int hydro_destroy(hydro_t *h)
 {
     if (!h) return fail(HYDRO_ERR_ARG, "destroy: NULL handle%s%s");
     cudaStreamSynchronize(h->stream);
+    drop_graph(h);
     for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
     for (auto e : h->pool) cudaEventDestroy(e);
     dev_free(h, h->block);
@@ -362,6 +424,7 @@ int hydro_set_stream(hydro_t *h, void *s)
 {
     if (!h) return fail(HYDRO_ERR_ARG, "set_stream: NULL handle%s%s");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
+    drop_graph(h);
     h->stream = (cudaStream_t)s;
     return HYDRO_OK;
 }
@@ -370,6 +433,7 @@ int hydro_set_cfl(hydro_t *h, double cfl)
 {
     if (!h || !(cfl > 0.0) || !std::isfinite(cfl)) return fail(HYDRO_ERR_ARG, "set_cfl: cfl must be > 0%s%s");
     h->cfl = cfl;
+    drop_graph(h);
     return HYDRO_OK;
 }
 
@@ -378,6 +442,7 @@ int hydro_set_limiter_theta(hydro_t *h, double theta)
     if (!h || !(theta >= 1.0 && theta <= 2.0))
         return fail(HYDRO_ERR_ARG, "set_limiter_theta: theta must be in [1,2]%s%s");
     h->g.theta = theta;
+    drop_graph(h);
     return HYDRO_OK;
 }
 
@@ -385,6 +450,7 @@ int hydro_set_kernel_variant(hydro_t *h, int variant)
 {
     if (!h || variant < 0 || variant > 1) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0 or 1%s%s");
     h->variant = variant;
+    drop_graph(h);
     return HYDRO_OK;
 }
 
@@ -479,22 +545,13 @@ int hydro_run_steps(hydro_t *h, long long n)
     if (n == 0) return HYDRO_OK;
     int rc;
     if (!h->smax_valid && (rc = launch_cfl_reduce(h))) return rc;
-    if (!h->t_on_device) {
-        begin_run_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->t);
-        LAUNCH_CHECK("begin_run");
-        h->t_on_device = true;
-    }
-    for (long long s = 0; s < n; ++s) {
-        {
-            Scope sc(h, K_NEXTDT);
-            next_dt_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->cfl, h->dx);
-        }
-        LAUNCH_CHECK("next_dt");
-        if ((rc = enqueue_step(h, 0.0, true))) return rc;
-    }
-    return HYDRO_OK;
+    if (!h->t_on_device && (rc = begin_run(h, HUGE_VAL))) return rc;
+    return enqueue_device_steps(h, n);
 }
 
+// Algorithm 1's while loop with the time step kept on the device: batches of steps are enqueued
+// without a host round trip; the kernel that forms dt clips the last step onto t_final and turns
+// any step enqueued beyond it into the identity, so the host only reads the scalars once per batch.
 int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
 {
     if (!h || !std::isfinite(t_final)) return fail(HYDRO_ERR_ARG, "evolve: bad argument%s%s");
@@ -502,18 +559,31 @@ int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
     int rc;
     if (h->t_on_device && (rc = read_scalars(h))) return rc;
     if (t_final < h->t) return fail(HYDRO_ERR_ARG, "evolve: t_final is in the past%s%s");
-    long long n = 0;
-    while (h->t < t_final) {
-        double dt;
-        if ((rc = hydro_cfl_dt(h, &dt))) return rc;
-        bool last = false;
-        if (h->t + dt >= t_final) { dt = t_final - h->t; last = true; }
-        if ((rc = hydro_step(h, dt))) return rc;
-        if (last) h->t = t_final;
-        ++n;
+    if (nsteps) *nsteps = 0;
+    if (!(h->t < t_final)) return HYDRO_OK;
+    if (!h->smax_valid && (rc = launch_cfl_reduce(h))) return rc;
+    if ((rc = begin_run(h, t_final))) return rc;
+    long long batch = 4;
+    for (;;) {
+        if ((rc = enqueue_device_steps(h, batch))) return rc;
+        CUDA_TRY(cudaMemcpyAsync(h->scal_host, h->scal, sizeof(StepScalars), cudaMemcpyDeviceToHost,
+                                 h->stream));
+        CUDA_TRY(cudaStreamSynchronize(h->stream));
+        const StepScalars &sc = *h->scal_host;
+        if (sc.flag) {
+            h->t = sc.t; h->step += sc.steps; h->t_on_device = false;
+            return fail(HYDRO_ERR_UNPHYSICAL, "unphysical state (rho<=0, p<=0 or non-finite speed)%s%s");
+        }
+        if (sc.done) break;
+        // size the next batch from the time left and the last dt (wasted identity steps are cheap
+        // but not free); never more than 64 steps between host checks
+        const double left = (t_final - sc.t) / (sc.dt > 0.0 ? sc.dt : 1.0);
+        batch = left < 1.0 ? 1 : (left > 64.0 ? 64 : (long long)left + 1);
     }
-    CUDA_TRY(cudaStreamSynchronize(h->stream));
-    if (nsteps) *nsteps = n;
+    h->t = h->scal_host->t;                       // == t_final exactly
+    h->step += h->scal_host->steps;
+    h->t_on_device = false;
+    if (nsteps) *nsteps = h->scal_host->steps;
     return HYDRO_OK;
 }
 

@@ -141,30 +141,43 @@ cfl_reduce_kernel(Grid g, const double *__restrict__ U, unsigned long long *smax
     block_max_to_global(s, bad, smax_bits, flag);
 }
 
-// Device-resident time step (hydro_run_steps): dt = (cfl/3) * (dx / smax); t += dt.
+// Device-resident time step (hydro_run_steps, hydro_evolve): dt = (cfl/3) * (dx / smax), clipped to
+// land on t_final exactly (O8 / R14); once t_final is reached further steps get dt = 0, which the
+// stage kernels turn into the identity (U + (-(0*D)) = U, 0.5*((U+U)+(-0)) = U, bit for bit).
 struct StepScalars {
     unsigned long long smax_bits;   // running max of the CFL reduction (bit pattern)
     int flag;                       // sticky: unphysical state seen
-    int pad;
+    int done;                       // t has reached t_final
     double dt;                      // time step of the current step
-    double t;                       // simulation time (device copy, used by run_steps)
-    long long steps;                // steps taken by run_steps since begin
+    double t;                       // simulation time (device copy)
+    long long steps;                // steps taken since begin_run
+    double t_final;                 // +inf for hydro_run_steps
 };
 
-__global__ void begin_run_kernel(StepScalars *s, double t0)
+__global__ void begin_run_kernel(StepScalars *s, double t0, double t_final)
 {
     s->t = t0;
     s->steps = 0;
+    s->t_final = t_final;
+    s->done = 0;
 }
 
 __global__ void next_dt_kernel(StepScalars *s, double cfl, double dx)
 {
+    if (s->done) { s->dt = 0.0; return; }
     const double smax = __longlong_as_double((long long)s->smax_bits);
     const double c3 = cfl / 3.0;
     const double dxs = dx / smax;
-    const double dt = c3 * dxs;
+    double dt = __dmul_rn(c3, dxs);                    // never contracted: same roundings on every build
+    const double t = s->t;
+    if (__dadd_rn(t, dt) >= s->t_final) {
+        dt = s->t_final - t;
+        s->t = s->t_final;
+        s->done = 1;
+    } else {
+        s->t = __dadd_rn(t, dt);
+    }
     s->dt = dt;
-    s->t = s->t + dt;
     s->steps += 1;
 }
 
