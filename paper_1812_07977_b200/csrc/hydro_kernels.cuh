@@ -33,20 +33,20 @@ __device__ __forceinline__ long long cell(const Grid &g, int I, int J, int K)
 __global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
                                   unsigned long long *__restrict__ clear_smax)
 {
-    const long long nxy = (long long)g.nx * g.ny, nyz = (long long)g.ny * g.nz,
-                    nzx = (long long)g.nz * g.nx;
-    long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // 32-bit index arithmetic (the three face counts are < 2^31 for any grid that fits the device)
+    const unsigned nxy = (unsigned)g.nx * g.ny, nyz = (unsigned)g.ny * g.nz, nzx = (unsigned)g.nz * g.nx;
+    unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t == 0 && clear_smax) *clear_smax = 0ull;
     int axis, n;
     long long base, stride;
     if (t < nxy) {                       // z faces: thread per (i,j), coalesced in i
-        const int i = (int)(t % g.nx), j = (int)(t / g.nx);
+        const int i = (int)(t % (unsigned)g.nx), j = (int)(t / (unsigned)g.nx);
         axis = 2; n = g.nz; base = cell(g, i + NG, j + NG, 0); stride = g.sy;
     } else if ((t -= nxy) < nzx) {       // y faces: thread per (i,k), coalesced in i
-        const int i = (int)(t % g.nx), k = (int)(t / g.nx);
+        const int i = (int)(t % (unsigned)g.nx), k = (int)(t / (unsigned)g.nx);
         axis = 1; n = g.ny; base = cell(g, i + NG, 0, k + NG); stride = g.px;
     } else if ((t -= nzx) < nyz) {       // x faces: thread per (j,k)
-        const int j = (int)(t % g.ny), k = (int)(t / g.ny);
+        const int j = (int)(t % (unsigned)g.ny), k = (int)(t / (unsigned)g.ny);
         axis = 0; n = g.nx; base = cell(g, 0, j + NG, k + NG); stride = 1;
     } else {
         return;

@@ -57,7 +57,11 @@ inline cudaError_t plan_stage_fused(FusedPlan &p, const Grid &g, const double *A
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     // tuning knobs (measurement only): HYDRO_FUSED_TY = 8 | 16, HYDRO_FUSED_LZ = planes per chunk
     const char *ety = getenv("HYDRO_FUSED_TY"), *elz = getenv("HYDRO_FUSED_LZ");
-    const int ty = (ety && atoi(ety) == 16) ? 16 : 8;
+    // 32 x 16 tiles (one 512-thread block per SM) carry half the per-warp halo / edge work of 32 x 8
+    // tiles (two 256-thread blocks per SM) and win on large grids (256^3: 1.615 vs 1.636 ms per
+    // step); small grids need the finer tiling to fill the machine
+    int ty = g.ny >= 128 ? 16 : 8;
+    if (ety) ty = atoi(ety) == 16 ? 16 : 8;
     int lz = fused_choose_lz(g, ty, nsm, ty == 16 ? 1 : 2);
     if (elz && atoi(elz) > 0) lz = atoi(elz);
     fused_geometry(p, g, ty, lz);
