@@ -235,6 +235,47 @@ def test_run_steps_equals_host_loop_bitwise_on_verification_build():
     assert g.get_time() == c.get_time()
 
 
+def test_graph_replay_is_rebuilt_when_parameters_change():
+    """hydro_run_steps replays a captured one-step graph; CFL, theta and the kernel variant are
+    baked into its launches, so changing them must rebuild it (verification build, bitwise)."""
+    shape = (40, 24, 20)
+    U = inputs.random_state(*shape, seed=21, vamp=0.3)
+    bc = (PER, PER, OUT, REF, REF, OUT)
+    g = _gpu(shape, 1.4, 1.0 / 40, bc, cfl=0.7, verify=True)
+    c = _cpu(shape, 1.4, 1.0 / 40, bc, cfl=0.7)
+    g.set_state(U); c.set_state(U)
+
+    def both(n):
+        g.run_steps(n)
+        for _ in range(n):
+            c.step(c.cfl_dt())
+        assert np.array_equal(g.get_state(), c.get_state())
+        assert g.get_time() == c.get_time()
+
+    both(3)
+    g.set_cfl(0.4); c.set_cfl(0.4); both(3)
+    g.set_limiter_theta(2.0); c.set_limiter_theta(2.0); both(2)
+    g.set_kernel_variant(0); both(2)
+    g.set_kernel_variant(1); both(2)
+
+
+def test_evolve_batches_land_on_t_final_with_identity_tail():
+    """hydro_evolve enqueues batches of device-dt steps; steps beyond t_final get dt = 0 and must
+    leave the state bit-identical.  Several t_final values so that the clipped step falls at
+    different places inside a batch; step counts and times must equal the oracle's."""
+    cfg = inputs.config(0)
+    U = cfg.state()
+    for t_final in (0.003, 0.02, 0.0475, 0.1):
+        g = _gpu(cfg.shape, cfg.gamma, cfg.dx, cfg.bc, cfg.cfl, verify=True)
+        c = _cpu(cfg.shape, cfg.gamma, cfg.dx, cfg.bc, cfg.cfl)
+        g.set_state(U); c.set_state(U)
+        ng, nc = g.evolve(t_final), c.evolve(t_final)
+        assert ng == nc and g.get_time() == c.get_time() == (t_final, nc)
+        assert np.array_equal(g.get_state(), c.get_state())
+        assert g.evolve(t_final) == 0                          # already there: no step
+        g.close()
+
+
 def test_config1_sod_evolve_to_t02():
     cfg = inputs.config(1)
     U = cfg.state()
