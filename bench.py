@@ -287,6 +287,20 @@ def run_ours(args):
                     "avg_launch_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in kt.items()},
                     "share_of_step": {k: v[0] / ms for k, v in kt.items()}}
 
+    # ---- the named ABI loop, state resident: K x (hydro_cfl_dt + hydro_step(dt)), i.e. one 32-byte
+    #      device->host read and a stream sync per step (SURVEY.md section 8(d) variant (i)) ----------
+    h.set_state(Ud)
+    for _ in range(3):
+        h.step(h.cfl_dt())
+    barrier()
+    ea0, ea1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ea0.record()
+    for _ in range(args.steps):
+        h.step(h.cfl_dt())
+    ea1.record()
+    torch.cuda.synchronize()
+    ms_abi = max_over_ranks(ea0.elapsed_time(ea1), world, "cuda")
+
     # ---- end to end through the C-ABI with HOST buffers --------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     Uh = U0.clone().pin_memory()
@@ -333,6 +347,9 @@ def run_ours(args):
                                          f"{world} independent replicas (no collective)",
                                          "dt": "device-resident (hydro_run_steps)"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+                "abi_loop": {"value": world * cells * args.steps / (ms_abi * 1e-3), "unit": UNIT,
+                             "ms_per_step": ms_abi / args.steps,
+                             "what": "K x (hydro_cfl_dt + hydro_step(dt)), state resident in HBM"},
                 "graph_replay": {"value": world * cells * args.steps / (ms_graph * 1e-3), "unit": UNIT,
                                  "ms_per_step": ms_graph / args.steps,
                                  "what": "same K steps without per-kernel events (CUDA-graph replay)"},
