@@ -353,7 +353,8 @@ def run_ours(args):
                 "graph_replay": {"value": world * cells * args.steps / (ms_graph * 1e-3), "unit": UNIT,
                                  "ms_per_step": ms_graph / args.steps,
                                  "what": "same K steps without per-kernel events (CUDA-graph replay)"},
-                "roofline": roofline, "cpu_baseline": cpu}
+                "roofline": roofline, "binding_roofline": "alu (fp64 pipe): see roofline_alu",
+                "cpu_baseline": cpu}
         if roofline:
             # fp64-pipe view of the same two launches: the kernel is bound
             # by the fp64 pipe, so this fraction, not the HBM one, says how close it is to the metal

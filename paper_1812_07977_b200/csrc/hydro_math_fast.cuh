@@ -44,11 +44,7 @@ __device__ __forceinline__ double rsqrt(double x)
 // sm_100a, measured; non-negative doubles order like their bit patterns)
 __device__ __forceinline__ double min_nonneg(double x, double y)
 {
-#ifdef HYD_MIN_FP64
-    return x < y ? x : y;
-#else
     return __double_as_longlong(x) < __double_as_longlong(y) ? x : y;
-#endif
 }
 
 __device__ __forceinline__ double max_nonneg(double x, double y)
@@ -78,14 +74,8 @@ __device__ __forceinline__ void limited_faces(double half_theta, const double Wm
     for (int v = 0; v < 5; ++v) {
         const double a = Wc[v] - Wm[v];
         const double b = Wp[v] - Wc[v];
-#ifdef HYD_LIMITER_INT
-        const long long ia = __double_as_longlong(a) & 0x7fffffffffffffffll, ib = __double_as_longlong(b) & 0x7fffffffffffffffll;
-        const double mn = __longlong_as_double(ia < ib ? ia : ib);
-        const double t1 = half_theta * mn;
-#else
-        const double mn = fabs(a) < fabs(b) ? a : b;
+        const double mn = fabs(a) < fabs(b) ? a : b;      // one DSETP; the integer form costs more issue slots
         const double t1 = half_theta * fabs(mn);
-#endif
         const double t2 = 0.25 * fabs(a + b);
         const double h = min_nonneg(t1, t2);
         const int ah = __double2hiint(a), bh = __double2hiint(b);

@@ -2,10 +2,6 @@
 #pragma once
 #include <cstdlib>
 
-#ifndef HYD_UNROLL_C
-#define HYD_UNROLL_C 1
-#endif
-
 namespace hyd {
 
 struct FusedArgs {
@@ -133,11 +129,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     }
     write_tile(Wa, sm + S::OFF_RING + 2 * S::STAGE, ty);      // cell plane 0 = raw plane 2; arrive_W(0)
 
-#if HYD_UNROLL_C == 2
-#pragma unroll 2
-#else
 #pragma unroll 1
-#endif
     for (int c = 0; c < nc; ++c) {
         const uint32_t par = c & 1;
         const int role = (ty + c) & (TY - 1);
