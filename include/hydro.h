@@ -82,7 +82,10 @@ int hydro_step(hydro_t *h, double dt);
 
 /* Algorithm 1 lines 3-4, 23: while t < t_final { dt = cfl_dt; clip the
  * last step to land on t_final exactly (R14); step }.  *nsteps (host, may be NULL) receives the
- * number of steps taken.  Synchronises.  HYDRO_ERR_ARG if t_final < t or non-finite. */
+ * number of steps taken.  The time step, the clipping and the clock stay on the device: steps are
+ * enqueued in batches (at most 64) between host reads of the device scalars, and a step enqueued
+ * past t_final runs with dt = 0, which leaves the state bit-identical.  Synchronises.
+ * HYDRO_ERR_ARG if t_final < t or non-finite; HYDRO_ERR_UNPHYSICAL as hydro_cfl_dt. */
 int hydro_evolve(hydro_t *h, double t_final, long long *nsteps);
 
 /* Copy the device state out into a packed array (host or device pointer).  Synchronises.
@@ -105,9 +108,10 @@ int hydro_set_stream(hydro_t *h, void *cuda_stream);
 int hydro_set_allocator(void *(*alloc)(size_t bytes, void *stream), void (*release)(void *ptr));
 /* n steps with the time step kept on the device: each step uses
  * dt = (cfl/3)*dx/smax with smax reduced by the previous step's last kernel (or by a
- * stand-alone reduction after set_state).  No host round trip; asynchronous.  The benchmark
- * path (Algorithm 1's loop body without the host-side ComputeTimeStep of Algorithm 2,
- * PAPER.md:198). */
+ * stand-alone reduction after set_state).  No host round trip; asynchronous.  On a non-default
+ * stream the step is captured once as a CUDA graph and replayed (rebuilt when the stream, CFL,
+ * theta or the kernel variant changes).  The benchmark path (Algorithm 1's loop body without the
+ * host-side ComputeTimeStep of Algorithm 2). */
 int hydro_run_steps(hydro_t *h, long long n);
 /* Test hooks: run only the ghost fill on the current state, and read the padded buffer
  * [5][nz+4][ny+4][nx+4] (x fastest, row pitch removed) into a host or device array. */
