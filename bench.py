@@ -5,7 +5,9 @@
 
 A "step" is one pass of the whole hot path (ghost fill, stage 1, ghost fill, stage 2 with fused
 CFL reduction, device-side dt) over the whole grid.  `value` is timed with CUDA events on the
-library's stream with the state already resident in HBM (hydro_run_steps); `e2e` is the same step
+library's stream with the state already resident in HBM (hydro_run_steps, CUDA-graph replay); per-kernel
+times for the roofline come from a second pass of the same steps with every launch bracketed by
+events; `e2e` is the same step
 through the C-ABI with HOST buffers: every timed step copies the state host->device
 (hydro_set_state from pinned memory), runs hydro_cfl_dt + hydro_step, and copies it back
 (hydro_get_state) -- the transfer pattern of the paper's Algorithm 2.
@@ -227,11 +229,12 @@ def run_ours(args):
     torch.cuda.synchronize()
 
     # ---- device-resident timing: K steps, state in HBM, device-side dt -----------------------
+    # Timed region = hydro_run_steps(K) as a user gets it (replay of the captured one-step CUDA
+    # graph), bracketed by CUDA events on the library's stream.
     h.set_state(Ud)
     h.run_steps(args.warmup)
     h.set_state(Ud)                                        # same physical state every run
     h.run_steps(max(args.warmup, 3))
-    L.hydro_set_profiling(h._h, 1)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
@@ -240,9 +243,9 @@ def run_ours(args):
     n0 = h.launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     tw0 = time.perf_counter()
-    ev0.record()
+    ev0.record(h.torch_stream)
     h.run_steps(args.steps)
-    ev1.record()
+    ev1.record(h.torch_stream)
     torch.cuda.synchronize()
     tw1 = time.perf_counter()
     barrier()
@@ -251,8 +254,17 @@ def run_ours(args):
     ms = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
     value = world * cells * args.steps / (ms * 1e-3)
 
-    # per-kernel durations recorded by the library with CUDA events on its own stream
+    # ---- the same K steps again with every kernel launch bracketed by CUDA events on the library's
+    #      stream (direct launches instead of graph replay): per-kernel durations for the roofline
     import ctypes as C
+    L.hydro_set_profiling(h._h, 1)
+    barrier()
+    eg0, eg1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    eg0.record(h.torch_stream)
+    h.run_steps(args.steps)
+    eg1.record(h.torch_stream)
+    torch.cuda.synchronize()
+    ms_prof = max_over_ranks(eg0.elapsed_time(eg1), world, "cuda")
     kt = {}
     for which, name in ((0, "ghost_fill"), (1, "stage1"), (2, "stage2"), (3, "next_dt")):
         tms, cnt = C.c_double(), C.c_longlong()
@@ -260,16 +272,6 @@ def run_ours(args):
         kt[name] = (tms.value, cnt.value)
     L.hydro_set_profiling(h._h, 0)
     _, nsteps = h.get_time()
-    # same K steps once more without per-kernel events: hydro_run_steps then replays its captured
-    # one-step CUDA graph (the path a user gets); reported beside `value`, which keeps the events
-    h.run_steps(3)
-    barrier()
-    eg0, eg1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    eg0.record()
-    h.run_steps(args.steps)
-    eg1.record()
-    torch.cuda.synchronize()
-    ms_graph = max_over_ranks(eg0.elapsed_time(eg1), world, "cuda")
     st_ms = kt["stage1"][0] + kt["stage2"][0]
     st_n = kt["stage1"][1] + kt["stage2"][1]
     roofline = None
@@ -285,7 +287,9 @@ def run_ours(args):
                     "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
                                                      "stage2": BYTES_STAGE[2] * cells},
                     "avg_launch_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in kt.items()},
-                    "share_of_step": {k: v[0] / ms for k, v in kt.items()}}
+                    "share_of_step": {k: v[0] / ms_prof for k, v in kt.items()},
+                    "timed_in": "second pass of the same K steps with per-kernel CUDA events on the "
+                                "library's stream (direct launches), %.4f ms per step" % (ms_prof / args.steps)}
 
     # ---- the named ABI loop, state resident: K x (hydro_cfl_dt + hydro_step(dt)), i.e. one 32-byte
     #      device->host read and a stream sync per step (SURVEY.md section 8(d) variant (i)) ----------
@@ -294,10 +298,10 @@ def run_ours(args):
         h.step(h.cfl_dt())
     barrier()
     ea0, ea1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ea0.record()
+    ea0.record(h.torch_stream)
     for _ in range(args.steps):
         h.step(h.cfl_dt())
-    ea1.record()
+    ea1.record(h.torch_stream)
     torch.cuda.synchronize()
     ms_abi = max_over_ranks(ea0.elapsed_time(ea1), world, "cuda")
 
@@ -345,14 +349,11 @@ def run_ours(args):
                 "data": "synthetic",
                 "config": cfg_dict(cfg, {"parallelism": "single GPU" if world == 1 else
                                          f"{world} independent replicas (no collective)",
-                                         "dt": "device-resident (hydro_run_steps)"}),
+                                         "dt": "device-resident (hydro_run_steps, CUDA-graph replay)"}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                 "abi_loop": {"value": world * cells * args.steps / (ms_abi * 1e-3), "unit": UNIT,
                              "ms_per_step": ms_abi / args.steps,
                              "what": "K x (hydro_cfl_dt + hydro_step(dt)), state resident in HBM"},
-                "graph_replay": {"value": world * cells * args.steps / (ms_graph * 1e-3), "unit": UNIT,
-                                 "ms_per_step": ms_graph / args.steps,
-                                 "what": "same K steps without per-kernel events (CUDA-graph replay)"},
                 "roofline": roofline, "binding_roofline": "alu (fp64 pipe): see roofline_alu",
                 "cpu_baseline": cpu}
         if roofline:

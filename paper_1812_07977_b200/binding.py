@@ -134,8 +134,15 @@ class Hydro:
         self._h = C.c_void_p()
         arr = (C.c_int * 6)(*[int(b) for b in bc])
         self._chk(self._L.hydro_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "hydro_create")
+        # The library enqueues on one stream.  By default that is a torch stream of the handle's own:
+        # torch's default stream is the legacy stream 0, which cannot be captured, and
+        # hydro_run_steps / hydro_evolve replay a captured CUDA graph.  Device tensors handed to
+        # set_state are ordered after the caller's current stream; get_state synchronises.
         if stream is None:
-            stream = torch.cuda.current_stream().cuda_stream
+            self.torch_stream = torch.cuda.Stream()
+            stream = self.torch_stream.cuda_stream
+        else:
+            self.torch_stream = torch.cuda.ExternalStream(int(stream)) if int(stream) else torch.cuda.default_stream()
         self._chk(self._L.hydro_set_stream(self._h, C.c_void_p(stream)), "hydro_set_stream")
 
     def _chk(self, rc, where):
@@ -163,17 +170,28 @@ class Hydro:
         self._chk(self._L.hydro_set_kernel_variant(self._h, variant), "hydro_set_kernel_variant")
 
     def set_stream(self, cuda_stream):
+        import torch
         self._chk(self._L.hydro_set_stream(self._h, C.c_void_p(cuda_stream)), "hydro_set_stream")
+        self.torch_stream = (torch.cuda.ExternalStream(int(cuda_stream)) if int(cuda_stream)
+                             else torch.cuda.default_stream())
 
     def set_state(self, U):
-        p, keep, _ = _as_ptr(U, self.shape)
+        import torch
+        p, keep, on_device = _as_ptr(U, self.shape)
+        if on_device:                                  # producer of U ran on the caller's stream
+            self.torch_stream.wait_stream(torch.cuda.current_stream())
+            U.record_stream(self.torch_stream)
         self._chk(self._L.hydro_set_state(self._h, p), "hydro_set_state")
 
     def get_state(self, out=None):
         if out is None:
             out = np.empty(self.shape)
-        p, keep, _ = _as_ptr(out, self.shape, writable=True)
-        self._chk(self._L.hydro_get_state(self._h, p), "hydro_get_state")
+        import torch
+        p, keep, on_device = _as_ptr(out, self.shape, writable=True)
+        if on_device:                                  # earlier users of `out` ran on the caller's stream
+            self.torch_stream.wait_stream(torch.cuda.current_stream())
+            out.record_stream(self.torch_stream)
+        self._chk(self._L.hydro_get_state(self._h, p), "hydro_get_state")   # synchronises
         return out
 
     def get_padded(self):

@@ -396,6 +396,8 @@ int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6
     if (e == cudaSuccess) e = cudaMemset(h->block, 0, 2 * h->buf_doubles * sizeof(double));
     if (e == cudaSuccess) e = cudaMemset(h->scal, 0, sizeof(StepScalars));
     if (e == cudaSuccess) e = plan_stage_fused(h->plan, g, h->A, h->B);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();   // the memsets ran on the legacy stream; the handle's
+                                                         // stream may be a non-blocking one
     if (e != cudaSuccess) {
         cudaGetLastError();
         fail(HYDRO_ERR_CUDA, "create: %s%s", cudaGetErrorString(e));
