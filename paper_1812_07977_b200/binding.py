@@ -92,7 +92,10 @@ def use_torch_allocator(L):
             return None
 
     def _free(ptr):
-        torch.cuda.caching_allocator_delete(int(ptr))
+        try:
+            torch.cuda.caching_allocator_delete(int(ptr))
+        except Exception:                      # interpreter shutdown: torch is already torn down
+            pass
 
     a, f = _ALLOC_T(_alloc), _FREE_T(_free)
     _hooks[key] = (a, f)                      # keep the callbacks alive
