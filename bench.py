@@ -388,10 +388,13 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per stage-pair launch from the committed ncu --set full capture")
     args = ap.parse_args()
-    if args.traffic is None:
-        p = os.path.join(ROOT, "profiles", "traffic.json")
+    if args.traffic is None:                  # committed ncu --set full capture (DRAM bytes per stage pair)
+        p = os.path.join(ROOT, "profiles", "r1_traffic.txt")
         if os.path.exists(p):
-            args.traffic = json.load(open(p)).get(f"config{args.config}")
+            for ln in open(p):
+                f = ln.split()
+                if len(f) == 2 and f[0] == f"config{args.config}":
+                    args.traffic = float(f[1])
     if args.impl == "reference":
         run_reference(args)
     else:
