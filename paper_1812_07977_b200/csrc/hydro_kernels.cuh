@@ -52,6 +52,30 @@ __global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
         return;
     }
     const int lo = g.bc[2 * axis], hi = g.bc[2 * axis + 1];
+    // x faces, fast path: the two ghost cells of a side are half of a 32-byte sector; storing the
+    // whole sector (the other half is row padding nobody reads) spares the DRAM a read-modify-write,
+    // and 16-byte vector accesses halve the instruction count.  Needs the sectors to line up
+    // (nx % 4 == 0; the first active cell of a row is 128-byte aligned) and >= 2 pad cells per row.
+    if (axis == 0 && (g.nx & 3) == 0 && g.px - (g.nx + 2 * NG) >= 2) {
+#pragma unroll
+        for (int v = 0; v < NVAR; ++v) {
+            double *a = U + v * g.sv + base;
+            const double sgn = (v == 1) ? -1.0 : 1.0;
+            const double2 l2 = *reinterpret_cast<const double2 *>(a + 2);       // cells 2, 3
+            const double2 h2 = *reinterpret_cast<const double2 *>(a + n);       // cells n, n+1
+            double2 gl, gh;
+            if (lo == 0)      { gl.x = l2.x; gl.y = l2.x; }
+            else if (lo == 1) { gl.x = sgn * l2.y; gl.y = sgn * l2.x; }
+            else              { gl = h2; }
+            if (hi == 0)      { gh.x = h2.y; gh.y = h2.y; }
+            else if (hi == 1) { gh.x = sgn * h2.y; gh.y = sgn * h2.x; }
+            else              { gh = l2; }
+            double2 *pl = reinterpret_cast<double2 *>(a - 2), *ph = reinterpret_cast<double2 *>(a + n + 2);
+            pl[0] = make_double2(0.0, 0.0); pl[1] = gl;
+            ph[0] = gh; ph[1] = make_double2(0.0, 0.0);
+        }
+        return;
+    }
 #pragma unroll
     for (int v = 0; v < NVAR; ++v) {
         double *a = U + v * g.sv + base;

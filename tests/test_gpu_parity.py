@@ -86,7 +86,9 @@ BCS = [(OUT,) * 6, (PER,) * 6, (REF,) * 6, (OUT, REF, PER, PER, REF, OUT),
 
 
 @pytest.mark.parametrize("bc", BCS)
-@pytest.mark.parametrize("shape", [(5, 4, 3), (37, 9, 6), (2, 2, 2)])
+@pytest.mark.parametrize("shape", [(5, 4, 3), (37, 9, 6), (2, 2, 2),
+                                   (40, 6, 5), (28, 3, 3),    # x faces: full-sector vector path
+                                   (12, 5, 4)])               # nx % 4 == 0 but no row padding
 def test_ghost_fill_bit_exact(bc, shape):
     nx, ny, nz = shape
     U = inputs.random_state(nx, ny, nz, seed=7)
