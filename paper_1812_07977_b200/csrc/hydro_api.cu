@@ -141,7 +141,7 @@ int launch_ghost_fill(hydro *h, double *U, bool clear_smax)
     const long long n = (long long)g.nx * g.ny + (long long)g.ny * g.nz + (long long)g.nz * g.nx;
     const int tb = 128;
     Scope sc(h, K_GHOST);
-    ghost_fill_kernel<<<(unsigned)((n + tb - 1) / tb), tb, 0, h->stream>>>(
+    ghost_fill_kernel<<<dim3((unsigned)((n + tb - 1) / tb), NVAR), tb, 0, h->stream>>>(
         g, U, clear_smax ? &h->scal->smax_bits : nullptr);
     LAUNCH_CHECK("ghost_fill");
     return HYDRO_OK;
