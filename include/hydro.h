@@ -123,7 +123,8 @@ int hydro_set_kernel_variant(hydro_t *h, int variant);
 /* Measurement hooks (bench.py): when enabled, every kernel launch of this handle is bracketed by
  * CUDA events on the handle's stream.  hydro_get_kernel_time synchronises and returns the summed
  * duration (ms) and launch count since profiling was enabled, for which = 0 ghost fill,
- * 1 stage-1 kernel, 2 stage-2 kernel, 3 next-dt kernel, 4 stand-alone CFL reduction. */
+ * 1 stage-1 kernel, 2 stage-2 kernel, 3 (unused: the time-step update is folded into the first ghost fill
+ * of a device-dt step), 4 stand-alone CFL reduction. */
 int hydro_set_profiling(hydro_t *h, int enable);
 int hydro_get_kernel_time(hydro_t *h, int which, double *ms, long long *count);
 /* Number of kernels this library has launched since load (for bench.py's gpu_launches). */

@@ -135,14 +135,14 @@ int is_device_pointer(const void *p, bool *on_device)
     return HYDRO_OK;
 }
 
-int launch_ghost_fill(hydro *h, double *U, bool clear_smax)
+int launch_ghost_fill(hydro *h, double *U, bool clear_smax, bool advance_dt = false)
 {
     const Grid &g = h->g;
     const long long n = (long long)g.nx * g.ny + (long long)g.ny * g.nz + (long long)g.nz * g.nx;
     const int tb = 128;
     Scope sc(h, K_GHOST);
     ghost_fill_kernel<<<dim3((unsigned)((n + tb - 1) / tb), NVAR), tb, 0, h->stream>>>(
-        g, U, clear_smax ? &h->scal->smax_bits : nullptr);
+        g, U, clear_smax ? &h->scal->smax_bits : nullptr, advance_dt ? h->scal : nullptr, h->cfl, h->dx);
     LAUNCH_CHECK("ghost_fill");
     return HYDRO_OK;
 }
@@ -187,7 +187,8 @@ int enqueue_step(hydro *h, double dt_host, bool dev_dt)
 {
     const double r = dt_host / h->dx;
     int rc;
-    if ((rc = launch_ghost_fill(h, h->A, false))) return rc;
+    // device dt: the first fill of the step also forms dt = (cfl/3) dx / smax and advances the clock
+    if ((rc = launch_ghost_fill(h, h->A, false, dev_dt))) return rc;
     if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
     if ((rc = launch_ghost_fill(h, h->B, true))) return rc;
     if ((rc = launch_stage<2>(h, h->B, h->A, h->A, r, dev_dt, true))) return rc;
@@ -247,16 +248,6 @@ void drop_graph(hydro *h)
     if (h->step_graph) { cudaGraphExecDestroy(h->step_graph); h->step_graph = nullptr; }
 }
 
-int launch_next_dt(hydro *h)
-{
-    {
-        Scope sc(h, K_NEXTDT);
-        next_dt_kernel<<<1, 1, 0, h->stream>>>(h->scal, h->cfl, h->dx);
-    }
-    LAUNCH_CHECK("next_dt");
-    return HYDRO_OK;
-}
-
 // n device-dt steps: replays of the captured one-step graph when possible (not on the legacy
 // default stream, which cannot be captured, and not while per-kernel profiling is on).
 int enqueue_device_steps(hydro *h, long long n)
@@ -267,8 +258,7 @@ int enqueue_device_steps(hydro *h, long long n)
         const long long before = g_launches.load();
         cudaGraph_t graph = nullptr;
         CUDA_TRY(cudaStreamBeginCapture(h->stream, cudaStreamCaptureModeThreadLocal));
-        rc = launch_next_dt(h);
-        if (!rc) rc = enqueue_step(h, 0.0, true);
+        rc = enqueue_step(h, 0.0, true);
         cudaError_t e = cudaStreamEndCapture(h->stream, &graph);
         if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
         if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "graph capture: %s%s", cudaGetErrorString(e));
@@ -283,7 +273,6 @@ int enqueue_device_steps(hydro *h, long long n)
             CUDA_TRY(cudaGraphLaunch(h->step_graph, h->stream));
             g_launches.fetch_add(h->graph_kernels, std::memory_order_relaxed);
         } else {
-            if ((rc = launch_next_dt(h))) return rc;
             if ((rc = enqueue_step(h, 0.0, true))) return rc;
         }
     }

@@ -24,6 +24,50 @@ __device__ __forceinline__ long long cell(const Grid &g, int I, int J, int K)
     return (long long)I + (long long)g.px * J + g.sy * K;
 }
 
+// Device-resident time step (hydro_run_steps, hydro_evolve): dt = (cfl/3) * (dx / smax), clipped to
+// land on t_final exactly (O8 / R14); once t_final is reached further steps get dt = 0, which the
+// stage kernels turn into the identity (U + (-(0*D)) = U, 0.5*((U+U)+(-0)) = U, bit for bit).
+struct StepScalars {
+    unsigned long long smax_bits;   // running max of the CFL reduction (bit pattern)
+    int flag;                       // sticky: unphysical state seen
+    int done;                       // t has reached t_final
+    double dt;                      // time step of the current step
+    double t;                       // simulation time (device copy)
+    long long steps;                // steps taken since begin_run
+    double t_final;                 // +inf for hydro_run_steps
+};
+
+__global__ void begin_run_kernel(StepScalars *s, double t0, double t_final)
+{
+    s->t = t0;
+    s->steps = 0;
+    s->t_final = t_final;
+    s->done = 0;
+}
+
+__device__ __forceinline__ void advance_dt(StepScalars *s, double cfl, double dx)
+{
+    if (s->done) { s->dt = 0.0; return; }
+    const double smax = __longlong_as_double((long long)s->smax_bits);
+    const double c3 = cfl / 3.0;
+    const double dxs = dx / smax;
+    double dt = __dmul_rn(c3, dxs);                    // never contracted: same roundings on every build
+    const double t = s->t;
+    if (__dadd_rn(t, dt) >= s->t_final) {
+        dt = s->t_final - t;
+        s->t = s->t_final;
+        s->done = 1;
+    } else {
+        s->t = __dadd_rn(t, dt);
+    }
+    s->dt = dt;
+    s->steps += 1;
+}
+
+// stand-alone form (kept for tests / other drivers); the step driver folds advance_dt into the
+// first ghost fill of the step, one launch less
+__global__ void next_dt_kernel(StepScalars *s, double cfl, double dx) { advance_dt(s, cfl, dx); }
+
 // ------------------------------------------------------------------------------------------
 // A1 ghost fill (R9).  One thread per (face pair of one axis, transverse active cell); each
 // thread fills the 2+2 ghost cells of its line for all 5 variables.  The three axes are
@@ -31,8 +75,12 @@ __device__ __forceinline__ long long cell(const Grid &g, int I, int J, int K)
 // Thread 0 optionally clears the max-signal-speed accumulator for the stage that follows.
 // ------------------------------------------------------------------------------------------
 __global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
-                                  unsigned long long *__restrict__ clear_smax)
+                                  unsigned long long *__restrict__ clear_smax,
+                                  StepScalars *advance, double cfl, double dx)
 {
+    // first fill of a device-dt step: one thread also forms this step's dt (the stage kernels that
+    // read it are launched after this kernel)
+    if (advance && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) advance_dt(advance, cfl, dx);
     // 32-bit index arithmetic (the three face counts are < 2^31 for any grid that fits the device)
     const unsigned nxy = (unsigned)g.nx * g.ny, nyz = (unsigned)g.ny * g.nz, nzx = (unsigned)g.nz * g.nx;
     unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -165,46 +213,6 @@ cfl_reduce_kernel(Grid g, const double *__restrict__ U, unsigned long long *smax
         }
     }
     block_max_to_global(s, bad, smax_bits, flag);
-}
-
-// Device-resident time step (hydro_run_steps, hydro_evolve): dt = (cfl/3) * (dx / smax), clipped to
-// land on t_final exactly (O8 / R14); once t_final is reached further steps get dt = 0, which the
-// stage kernels turn into the identity (U + (-(0*D)) = U, 0.5*((U+U)+(-0)) = U, bit for bit).
-struct StepScalars {
-    unsigned long long smax_bits;   // running max of the CFL reduction (bit pattern)
-    int flag;                       // sticky: unphysical state seen
-    int done;                       // t has reached t_final
-    double dt;                      // time step of the current step
-    double t;                       // simulation time (device copy)
-    long long steps;                // steps taken since begin_run
-    double t_final;                 // +inf for hydro_run_steps
-};
-
-__global__ void begin_run_kernel(StepScalars *s, double t0, double t_final)
-{
-    s->t = t0;
-    s->steps = 0;
-    s->t_final = t_final;
-    s->done = 0;
-}
-
-__global__ void next_dt_kernel(StepScalars *s, double cfl, double dx)
-{
-    if (s->done) { s->dt = 0.0; return; }
-    const double smax = __longlong_as_double((long long)s->smax_bits);
-    const double c3 = cfl / 3.0;
-    const double dxs = dx / smax;
-    double dt = __dmul_rn(c3, dxs);                    // never contracted: same roundings on every build
-    const double t = s->t;
-    if (__dadd_rn(t, dt) >= s->t_final) {
-        dt = s->t_final - t;
-        s->t = s->t_final;
-        s->done = 1;
-    } else {
-        s->t = __dadd_rn(t, dt);
-    }
-    s->dt = dt;
-    s->steps += 1;
 }
 
 // ------------------------------------------------------------------------------------------
