@@ -17,8 +17,12 @@
 //     shared memory once; each thread computes the slopes of its own cell, hands its outer face
 //     value to the +x / +y neighbour through shared memory, computes the flux through its low
 //     face and hands that to the -x / -y neighbour's divergence.  The tile's extra high-edge
-//     faces and the two halo-cell slopes they need are a flattened list done by the first warps.
-//   * conserved state crosses HBM once per stage (interior planes; halos and the two warm-up
+//     faces and the two halo-cell slopes they need are a flattened list whose owner rotates over
+//     the warps from plane to plane.
+//   * the conserved planes (tile + halo, all five variables) arrive through a TMA ring
+//     (cp.async.bulk.tensor, one 4-D box per plane); the three hand-offs per plane are split-phase
+//     mbarriers with z-direction work between arrive and wait (see the kernel).
+//   * conserved state crosses HBM once per stage (interior planes; halos and the four extra
 //     planes per chunk re-read through L2).
 #pragma once
 #include "hydro_kernels.cuh"
