@@ -276,22 +276,33 @@ def run_ours(args):
     _, nsteps = h.get_time()
     st_ms = kt["stage1"][0] + kt["stage2"][0]
     st_n = kt["stage1"][1] + kt["stage2"][1]
-    roofline = None
+    roofline = roofline_hbm = None
     if st_n:
         bytes_pair = (BYTES_STAGE[1] + BYTES_STAGE[2]) * cells     # one stage-1 + one stage-2 launch
         avg_pair_ms = st_ms / (st_n / 2)
         achieved = bytes_pair / (avg_pair_ms * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                    "frac": achieved / hbm_peak, "traffic": args.traffic,
-                    "kernel": "stage_fused<1> + stage_fused<2> (one RK2 step's two stage launches)"
-                              if (args.variant is None or args.variant == 1) else "stage_simple<1,2>",
-                    "peak_source": peak_src,
-                    "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
-                                                     "stage2": BYTES_STAGE[2] * cells},
-                    "avg_launch_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in kt.items()},
-                    "share_of_step": {k: v[0] / ms_prof for k, v in kt.items()},
-                    "timed_in": "second pass of the same K steps with per-kernel CUDA events on the "
-                                "library's stream (direct launches), %.4f ms per step" % (ms_prof / args.steps)}
+        common = {"kernel": "stage_fused<1> + stage_fused<2> (one RK2 step's two stage launches)"
+                            if (args.variant is None or args.variant == 1) else "stage_simple<1,2>",
+                  "avg_launch_ms": {k: (v[0] / v[1] if v[1] else None) for k, v in kt.items()},
+                  "share_of_step": {k: v[0] / ms_prof for k, v in kt.items()},
+                  "timed_in": "second pass of the same K steps with per-kernel CUDA events on the "
+                              "library's stream (direct launches), %.4f ms per step" % (ms_prof / args.steps)}
+        # HBM view (BASELINE.json's metric): algorithmic bytes of the two stage launches / their time
+        roofline_hbm = dict({"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                             "frac": achieved / hbm_peak, "traffic": args.traffic,
+                             "peak_source": peak_src,
+                             "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
+                                                              "stage2": BYTES_STAGE[2] * cells}}, **common)
+        # fp64-pipe view of the same two launches: the roofline that BINDS this kernel (DESIGN.md
+        # section 6.1: 4.3 fp64 instructions per byte against a machine balance of 2.8)
+        peak = N_SM * FP64_LANES_PER_SM * sm_max * 1e6 / 1e12
+        ach = (FP64_INSTR_STAGE[1] + FP64_INSTR_STAGE[2]) * cells / (avg_pair_ms * 1e-3) / 1e12
+        roofline = dict({"bound": "alu", "achieved": ach, "peak": peak, "unit": "T fp64 thread-instr/s",
+                         "frac": ach / peak, "traffic": args.traffic_alu,
+                         "algorithmic_instr_per_cell": FP64_INSTR_STAGE,
+                         "peak_source": "63 fp64 lanes/clk/SM (measured DFMA/DADD/DMUL rate, "
+                                        "profiles/r1_fp64_pipe_microbench.md) x 148 SM x clocks.max.sm"},
+                        **common)
 
     # ---- the named ABI loop, state resident: K x (hydro_cfl_dt + hydro_step(dt)), i.e. one 32-byte
     #      device->host read and a stream sync per step (SURVEY.md section 8(d) variant (i)) ----------
@@ -356,19 +367,8 @@ def run_ours(args):
                 "abi_loop": {"value": world * cells * args.steps / (ms_abi * 1e-3), "unit": UNIT,
                              "ms_per_step": ms_abi / args.steps,
                              "what": "K x (hydro_cfl_dt + hydro_step(dt)), state resident in HBM"},
-                "roofline": roofline, "binding_roofline": "alu (fp64 pipe): see roofline_alu",
-                "cpu_baseline": cpu}
+                "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu}
         if roofline:
-            # fp64-pipe view of the same two launches: the kernel is bound
-            # by the fp64 pipe, so this fraction, not the HBM one, says how close it is to the metal
-            clk = (clocks or {}).get("sm_max_mhz") or sm_max
-            peak = N_SM * FP64_LANES_PER_SM * clk * 1e6 / 1e12
-            ach = (FP64_INSTR_STAGE[1] + FP64_INSTR_STAGE[2]) * cells / (avg_pair_ms * 1e-3) / 1e12
-            line["roofline_alu"] = {
-                "bound": "alu", "achieved": ach, "peak": peak, "unit": "T fp64 thread-instr/s",
-                "frac": ach / peak,
-                "algorithmic_instr_per_cell": FP64_INSTR_STAGE,
-                "peak_source": "63 fp64 lanes/clk/SM x 148 SM x clocks.max.sm (measured DFMA rate)"}
             line["hbm_gbs_whole_step"] = ((BYTES_STAGE[1] + BYTES_STAGE[2]) * cells * args.steps
                                           / (ms * 1e-3) / 1e9)
         print(json.dumps(line), flush=True)
@@ -390,13 +390,15 @@ def main():
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per stage-pair launch from the committed ncu --set full capture")
     args = ap.parse_args()
-    if args.traffic is None:                  # committed ncu --set full capture (DRAM bytes per stage pair)
-        p = os.path.join(ROOT, "profiles", "r1_traffic.txt")
-        if os.path.exists(p):
-            for ln in open(p):
-                f = ln.split()
-                if len(f) == 2 and f[0] == f"config{args.config}":
-                    args.traffic = float(f[1])
+    args.traffic_alu = None
+    p = os.path.join(ROOT, "profiles", "r1_traffic.txt")   # committed ncu --set full capture
+    if os.path.exists(p):
+        for ln in open(p):
+            f = ln.split()
+            if len(f) == 2 and f[0] == f"config{args.config}" and args.traffic is None:
+                args.traffic = float(f[1])                 # DRAM bytes per stage pair
+            if len(f) == 2 and f[0] == f"config{args.config}_fp64_executed":
+                args.traffic_alu = float(f[1])             # fp64 thread-instructions executed per stage pair
     if args.impl == "reference":
         run_reference(args)
     else:
