@@ -206,9 +206,18 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device and no CPU fallback")
+    # HYDRO_BENCH_BACKEND=gloo lets the N > 1 path (rendezvous, barriers, max-over-ranks timing) be
+    # exercised on a box with fewer GPUs than ranks: the replicas then share devices (they only meet
+    # at host-side barriers, no kernel waits on another rank)
+    backend = os.environ.get("HYDRO_BENCH_BACKEND", "nccl")
+    local = local % torch.cuda.device_count() if backend != "nccl" else local
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
+    red_dev = "cuda" if backend == "nccl" else "cpu"
 
     def barrier():
         if world > 1:
@@ -235,13 +244,13 @@ def run_ours(args):
     h.run_steps(args.warmup)
     h.set_state(Ud)                                        # same physical state every run
     h.run_steps(max(args.warmup, 3))
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
         t_wait = time.perf_counter()                       # nvidia-smi needs a moment to start
         while not sampler.rows and time.perf_counter() - t_wait < 3.0:
             time.sleep(0.02)
+    barrier()                                              # all ranks enter the timed region together
     n0 = h.launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     tw0 = time.perf_counter()
@@ -253,7 +262,7 @@ def run_ours(args):
     barrier()
     launches = h.launch_count() - n0
     clocks = sampler.stop(tw0, tw1) if rank == 0 else None
-    ms = max_over_ranks(ev0.elapsed_time(ev1), world, "cuda")
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world, red_dev)
     value = world * cells * args.steps / (ms * 1e-3)
 
     # ---- the same K steps again with every kernel launch bracketed by CUDA events on the library's
@@ -266,7 +275,7 @@ def run_ours(args):
     h.run_steps(args.steps)
     eg1.record(h.torch_stream)
     torch.cuda.synchronize()
-    ms_prof = max_over_ranks(eg0.elapsed_time(eg1), world, "cuda")
+    ms_prof = max_over_ranks(eg0.elapsed_time(eg1), world, red_dev)
     kt = {}
     for which, name in ((0, "ghost_fill"), (1, "stage1"), (2, "stage2"), (3, "next_dt")):
         tms, cnt = C.c_double(), C.c_longlong()
@@ -316,7 +325,7 @@ def run_ours(args):
         h.step(h.cfl_dt())
     ea1.record(h.torch_stream)
     torch.cuda.synchronize()
-    ms_abi = max_over_ranks(ea0.elapsed_time(ea1), world, "cuda")
+    ms_abi = max_over_ranks(ea0.elapsed_time(ea1), world, red_dev)
 
     # ---- end to end through the C-ABI with HOST buffers --------------------------------------
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
@@ -331,7 +340,7 @@ def run_ours(args):
         h.get_state(out_h)                                 # D2H of the step's result
         Uh, out_h = out_h, Uh
     torch.cuda.synchronize()
-    te = max_over_ranks(time.perf_counter() - te0, world, "cuda")
+    te = max_over_ranks(time.perf_counter() - te0, world, red_dev)
     state_bytes = 5 * cells * 8
     e2e = {"value": world * cells * e2e_steps / te, "unit": UNIT,
            "h2d_bytes_per_step": state_bytes, "d2h_bytes_per_step": state_bytes + 48,
@@ -347,7 +356,7 @@ def run_ours(args):
     for _ in range(args.steps):
         h.step(h.cfl_dt())
     h.get_state(out_h)
-    tj = max_over_ranks(time.perf_counter() - tj0, world, "cuda")
+    tj = max_over_ranks(time.perf_counter() - tj0, world, red_dev)
     e2e["job"] = {"value": world * cells * args.steps / tj, "unit": UNIT, "steps": args.steps,
                   "what": "hydro_set_state(host) once + K x (hydro_cfl_dt + hydro_step) + "
                           "hydro_get_state(host) once"}

@@ -49,3 +49,26 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank0():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["unit"] == "cell-updates/s"
     assert d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["e2e"]["d2h_bytes_per_step"] == 0
+
+
+import pytest
+
+
+@pytest.mark.gpu
+def test_ours_arm_two_ranks_share_one_gpu_over_gloo():
+    """The N > 1 path of bench.py end to end on whatever GPUs are present: two replica ranks
+    (HYDRO_BENCH_BACKEND=gloo lets them share a device; they meet only at host barriers), one
+    JSON line from rank 0 with the aggregate over both."""
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", "29613", "bench.py", "--gpus", "2",
+           "--config", "0", "--steps", "20", "--warmup", "3", "--e2e-steps", "1"]
+    env = dict(os.environ, HYDRO_BENCH_BACKEND="gloo", OMP_NUM_THREADS="2")
+    out = subprocess.run(cmd, cwd=ROOT, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE,
+                         text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and d["value"] > 0
+    assert d["config"]["parallelism"].startswith("2 independent replicas")
+    assert d["gpu_launches"] > 0 and d["cpu_baseline"] is None
