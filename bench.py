@@ -48,6 +48,44 @@ def max_over_ranks(x, world, device):
     return float(t.item())
 
 
+def csrc_sha256():
+    """Hash of the CUDA sources the library is built from: keys the committed ncu capture."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1812_07977_b200", "csrc")
+    hsh = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            hsh.update(f.encode())
+            hsh.update(open(os.path.join(d, f), "rb").read())
+    return hsh.hexdigest()[:16]
+
+
+def load_traffic(config):
+    """roofline.traffic comes from a committed `ncu --set full` capture (a bench run is never taken
+    under a profiler).  profiles/traffic.txt names the sources it was captured from (csrc_sha256);
+    a capture of other sources is refused, so the number cannot go stale silently."""
+    p = os.path.join(ROOT, "profiles", "traffic.txt")
+    out = {"dram": None, "fp64": None, "source": "no committed capture (profiles/traffic.txt absent)"}
+    if not os.path.exists(p):
+        return out
+    kv = {}
+    for ln in open(p):
+        f = ln.split()
+        if len(f) == 2 and not ln.startswith("#"):
+            kv[f[0]] = f[1]
+    have, want = kv.get("csrc_sha256"), csrc_sha256()
+    if have != want:
+        out["source"] = f"stale capture refused: profiles/traffic.txt is of csrc {have}, library is {want}"
+        return out
+    if f"config{config}" in kv:
+        out["dram"] = float(kv[f"config{config}"])
+    if f"config{config}_fp64_executed" in kv:
+        out["fp64"] = float(kv[f"config{config}_fp64_executed"])
+    out["source"] = (f"committed ncu --set full capture of csrc {have} "
+                     f"({kv.get('capture', 'profiles/')}), per stage-pair launch")
+    return out
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -226,6 +264,7 @@ def run_ours(args):
 
     cfg = workload(args.config)
     L = load_library(False)
+    traffic = load_traffic(args.config)
     hbm_peak, peak_src, sm_max = load_peaks()
     cells = cfg.cells
 
@@ -233,6 +272,9 @@ def run_ours(args):
     h.set_cfl(cfg.cfl)
     if args.variant is not None:
         h.set_kernel_variant(args.variant)
+    if args.tile_rows or args.planes_per_chunk:
+        h.set_tiling(args.tile_rows, args.planes_per_chunk)
+    tiling = h.get_tiling()
     U0 = torch.from_numpy(cfg.state()).pin_memory()        # pinned host copy of the input
     Ud = U0.cuda(non_blocking=True)
     torch.cuda.synchronize()
@@ -298,8 +340,9 @@ def run_ours(args):
                               "library's stream (direct launches), %.4f ms per step" % (ms_prof / args.steps)}
         # HBM view (BASELINE.json's metric): algorithmic bytes of the two stage launches / their time
         roofline_hbm = dict({"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                             "frac": achieved / hbm_peak, "traffic": args.traffic,
-                             "peak_source": peak_src,
+                             "frac": achieved / hbm_peak, "traffic": traffic["dram"],
+                             "traffic_source": traffic["source"], "peak_source": peak_src,
+                             "target": "north_star asks for >= 0.70 of peak HBM in the stage kernels",
                              "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
                                                               "stage2": BYTES_STAGE[2] * cells}}, **common)
         # fp64-pipe view of the same two launches: the roofline that BINDS this kernel (DESIGN.md
@@ -307,7 +350,12 @@ def run_ours(args):
         peak = N_SM * FP64_LANES_PER_SM * sm_max * 1e6 / 1e12
         ach = (FP64_INSTR_STAGE[1] + FP64_INSTR_STAGE[2]) * cells / (avg_pair_ms * 1e-3) / 1e12
         roofline = dict({"bound": "alu", "achieved": ach, "peak": peak, "unit": "T fp64 thread-instr/s",
-                         "frac": ach / peak, "traffic": args.traffic_alu,
+                         "frac": ach / peak, "traffic": traffic["fp64"],
+                         "traffic_source": traffic["source"],
+                         "note": "the kernel saturates neither roofline (latency / issue-slot "
+                                 "limited); both views are reported with equal standing: "
+                                 "roofline (fp64 pipe) and roofline_hbm (BASELINE.json's metric)",
+                         "hbm_frac": achieved / hbm_peak,
                          "algorithmic_instr_per_cell": FP64_INSTR_STAGE,
                          "peak_source": "63 fp64 lanes/clk/SM (measured DFMA/DADD/DMUL rate, "
                                         "profiles/r1_fp64_pipe_microbench.md) x 148 SM x clocks.max.sm"},
@@ -371,12 +419,18 @@ def run_ours(args):
                 "data": "synthetic",
                 "config": cfg_dict(cfg, {"parallelism": "single GPU" if world == 1 else
                                          f"{world} independent replicas (no collective)",
-                                         "dt": "device-resident (hydro_run_steps, CUDA-graph replay)"}),
+                                         "dt": "device-resident (hydro_run_steps, CUDA-graph replay)",
+                                         "stage_kernel_geometry": tiling}),
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
                 "abi_loop": {"value": world * cells * args.steps / (ms_abi * 1e-3), "unit": UNIT,
                              "ms_per_step": ms_abi / args.steps,
                              "what": "K x (hydro_cfl_dt + hydro_step(dt)), state resident in HBM"},
                 "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu}
+        n_dev = torch.cuda.device_count()
+        if backend != "nccl" or world > n_dev:
+            # replicas share devices (HYDRO_BENCH_BACKEND=gloo plumbing test): not a multi-GPU figure
+            line["devices_shared"] = True
+            line["distinct_devices"] = min(world, n_dev)
         if roofline:
             line["hbm_gbs_whole_step"] = ((BYTES_STAGE[1] + BYTES_STAGE[2]) * cells * args.steps
                                           / (ms * 1e-3) / 1e9)
@@ -396,18 +450,9 @@ def main():
     ap.add_argument("--variant", type=int, default=None)
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--traffic", type=float, default=None,
-                    help="dram bytes per stage-pair launch from the committed ncu --set full capture")
+    ap.add_argument("--tile-rows", type=int, default=0, help="hydro_set_tiling (0 = library's choice)")
+    ap.add_argument("--planes-per-chunk", type=int, default=0)
     args = ap.parse_args()
-    args.traffic_alu = None
-    p = os.path.join(ROOT, "profiles", "r1_traffic.txt")   # committed ncu --set full capture
-    if os.path.exists(p):
-        for ln in open(p):
-            f = ln.split()
-            if len(f) == 2 and f[0] == f"config{args.config}" and args.traffic is None:
-                args.traffic = float(f[1])                 # DRAM bytes per stage pair
-            if len(f) == 2 and f[0] == f"config{args.config}_fp64_executed":
-                args.traffic_alu = float(f[1])             # fp64 thread-instructions executed per stage pair
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -17,7 +17,10 @@
  *    variable order (rho, m_x, m_y, m_z, E) ("Value(nCells,nVariables)").
  *  - A `U` pointer may be a HOST pointer (pageable or pinned) or a DEVICE pointer on the
  *    handle's device; the library detects which (cudaPointerGetAttributes).  The caller owns
- *    `U` and may free or reuse it as soon as the call returns.
+ *    `U` and may free or reuse it as soon as the call returns (hydro_set_state and
+ *    hydro_get_state synchronise the handle's stream for host and device pointers alike; a device
+ *    `U` written by work on ANOTHER stream must be complete, or ordered before the handle's stream
+ *    by the caller, when the call is made).
  *  - The handle owns all device memory it allocates (two ghost-padded SoA buffers + scalars).
  *  - Work is enqueued on the handle's stream (default: the legacy default stream; see
  *    hydro_set_stream).  hydro_step / hydro_run_steps only enqueue; hydro_cfl_dt,
@@ -66,7 +69,7 @@ int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6
                  hydro_t **out);
 
 /* Copy a packed state (host or device pointer, layout above) into the device state; resets the
- * time to 0 and the step count to 0.  Synchronous for pageable host memory. */
+ * time to 0 and the step count to 0.  Synchronises the handle's stream. */
 int hydro_set_state(hydro_t *h, const double *U);
 
 /* Algorithm 1 line 5, "ComputeTimeStep": reduction over active cells,
@@ -84,8 +87,11 @@ int hydro_step(hydro_t *h, double dt);
  * last step to land on t_final exactly (R14); step }.  *nsteps (host, may be NULL) receives the
  * number of steps taken.  The time step, the clipping and the clock stay on the device: steps are
  * enqueued in batches (at most 64) between host reads of the device scalars, and a step enqueued
- * past t_final runs with dt = 0, which leaves the state bit-identical.  Synchronises.
- * HYDRO_ERR_ARG if t_final < t or non-finite; HYDRO_ERR_UNPHYSICAL as hydro_cfl_dt. */
+ * past t_final runs with dt = 0, which leaves the state numerically identical (U + 0 and
+ * 0.5*((U + U) + 0): every value keeps its bits except that a conserved value of -0.0 may come back
+ * as +0.0).  Synchronises.
+ * HYDRO_ERR_ARG if t_final < t or non-finite; HYDRO_ERR_UNPHYSICAL as hydro_cfl_dt, and when the
+ * time step stops advancing the clock (dt underflows to 0 or t + dt == t). */
 int hydro_evolve(hydro_t *h, double t_final, long long *nsteps);
 
 /* Copy the device state out into a packed array (host or device pointer).  Synchronises.
@@ -117,6 +123,15 @@ int hydro_run_steps(hydro_t *h, long long n);
  * [5][nz+4][ny+4][nx+4] (x fastest, row pitch removed) into a host or device array. */
 int hydro_ghost_fill(hydro_t *h);
 int hydro_get_padded(hydro_t *h, double *Upad);
+/* Tuning hooks of the fused stage kernel (tests and measurement; defaults are chosen per grid).
+ * hydro_set_tiling: tile_rows = 8 | 16 (rows of 32 cells per block; 0 = chosen by the library),
+ * planes_per_chunk = z-planes a block marches over (0 = chosen so that the blocks fill whole waves
+ * of the SMs).  hydro_get_tiling reports the geometry in use and the number of blocks per stage
+ * launch (any out-pointer may be NULL).  hydro_set_graph_replay(h, 0) makes hydro_run_steps /
+ * hydro_evolve enqueue plain launches instead of replaying the captured one-step CUDA graph. */
+int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk);
+int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long long *blocks);
+int hydro_set_graph_replay(hydro_t *h, int enable);
 /* Select the stage-kernel implementation: 0 = reference-structured simple kernel
  * (one thread per cell, everything recomputed), 1 = fused tiled kernel (default). */
 int hydro_set_kernel_variant(hydro_t *h, int variant);

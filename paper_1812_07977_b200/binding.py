@@ -20,7 +20,9 @@ SYMBOLS = ["hydro_create", "hydro_set_state", "hydro_cfl_dt", "hydro_step", "hyd
            "hydro_get_state", "hydro_destroy", "hydro_set_cfl", "hydro_set_limiter_theta",
            "hydro_get_time", "hydro_max_signal_speed", "hydro_set_stream", "hydro_set_allocator",
            "hydro_run_steps", "hydro_ghost_fill", "hydro_get_padded", "hydro_set_kernel_variant",
-           "hydro_set_profiling", "hydro_get_kernel_time", "hydro_launch_count", "hydro_is_verification_build", "hydro_last_error"]
+           "hydro_set_tiling", "hydro_get_tiling", "hydro_set_graph_replay",
+           "hydro_set_profiling", "hydro_get_kernel_time", "hydro_launch_count",
+           "hydro_is_verification_build", "hydro_last_error"]
 
 
 class HydroError(RuntimeError):
@@ -69,6 +71,9 @@ def load_library(verify=False):
     L.hydro_run_steps.argtypes = [vp, C.c_longlong]
     L.hydro_ghost_fill.argtypes = [vp]
     L.hydro_set_kernel_variant.argtypes = [vp, C.c_int]
+    L.hydro_set_tiling.argtypes = [vp, C.c_int, C.c_int]
+    L.hydro_get_tiling.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
+    L.hydro_set_graph_replay.argtypes = [vp, C.c_int]
     L.hydro_set_profiling.argtypes = [vp, C.c_int]
     L.hydro_get_kernel_time.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_longlong)]
     L.hydro_launch_count.restype = C.c_longlong
@@ -78,11 +83,22 @@ def load_library(verify=False):
     return L
 
 
-def use_torch_allocator(L):
-    """Install torch's caching allocator as the library's device-memory hook."""
+def use_torch_allocator(L, enable=True):
+    """Install torch's caching allocator as the library's (process-wide) device-memory hook, or
+    restore cudaMalloc / cudaFree with enable=False.  Called around every hydro_create, so that the
+    choice is per handle (a handle remembers the release function it was allocated with)."""
     import torch
     key = id(L)
+    if not enable:
+        rc = L.hydro_set_allocator(None, None)
+        if rc:
+            raise HydroError(rc, "hydro_set_allocator", L.hydro_last_error().decode())
+        return
     if key in _hooks:
+        a, f = _hooks[key]
+        rc = L.hydro_set_allocator(C.cast(a, C.c_void_p), C.cast(f, C.c_void_p))
+        if rc:
+            raise HydroError(rc, "hydro_set_allocator", L.hydro_last_error().decode())
         return
 
     def _alloc(nbytes, stream):
@@ -129,9 +145,8 @@ class Hydro:
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: this library has no CPU fallback")
         self._L = load_library(verify)
-        if torch_allocator:
-            torch.cuda.init()
-            use_torch_allocator(self._L)
+        torch.cuda.init()
+        use_torch_allocator(self._L, bool(torch_allocator))
         self.shape = (5, nz, ny, nx)
         self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
         self._h = C.c_void_p()
@@ -171,6 +186,18 @@ class Hydro:
 
     def set_kernel_variant(self, variant):
         self._chk(self._L.hydro_set_kernel_variant(self._h, variant), "hydro_set_kernel_variant")
+
+    def set_tiling(self, tile_rows=0, planes_per_chunk=0):
+        self._chk(self._L.hydro_set_tiling(self._h, tile_rows, planes_per_chunk), "hydro_set_tiling")
+
+    def get_tiling(self):
+        ty, lz, nb = C.c_int(), C.c_int(), C.c_longlong()
+        self._chk(self._L.hydro_get_tiling(self._h, C.byref(ty), C.byref(lz), C.byref(nb)),
+                  "hydro_get_tiling")
+        return {"tile": [32, ty.value], "planes_per_chunk": lz.value, "blocks": nb.value}
+
+    def set_graph_replay(self, enable):
+        self._chk(self._L.hydro_set_graph_replay(self._h, int(bool(enable))), "hydro_set_graph_replay")
 
     def set_stream(self, cuda_stream):
         import torch

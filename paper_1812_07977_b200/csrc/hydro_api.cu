@@ -63,6 +63,8 @@ struct hydro {
     double t = 0.0;
     long long step = 0;
     int variant = 1;
+    bool graph_replay = true;       // hydro_set_graph_replay
+    int ty_req = 0, lz_req = 0;     // hydro_set_tiling (0 = chosen by the library)
     FusedPlan plan;                 // launch geometry / TMA descriptors of the fused kernel
     // one device-dt RK2 step (next_dt + stage launches) captured as a CUDA graph, replayed by
     // hydro_run_steps / hydro_evolve; rebuilt when anything baked into the launches changes
@@ -83,9 +85,9 @@ enum { K_GHOST = 0, K_STAGE1 = 1, K_STAGE2 = 2, K_NEXTDT = 3, K_CFL = 4 };
 
 cudaEvent_t take_event(hydro *h)
 {
-    cudaEvent_t e;
+    cudaEvent_t e = nullptr;
     if (!h->pool.empty()) { e = h->pool.back(); h->pool.pop_back(); return e; }
-    cudaEventCreate(&e);
+    if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
     return e;
 }
 
@@ -94,11 +96,15 @@ struct Scope {
     hydro *h; int which; cudaEvent_t a = nullptr;
     Scope(hydro *h_, int w) : h(h_), which(w)
     {
-        if (h->profiling) { a = take_event(h); cudaEventRecord(a, h->stream); }
+        if (h->profiling && (a = take_event(h))) cudaEventRecord(a, h->stream);
     }
     ~Scope()
     {
-        if (a) { cudaEvent_t b = take_event(h); cudaEventRecord(b, h->stream); h->spans.push_back({which, a, b}); }
+        if (!a) return;                            // profiling off, or no event to be had: span dropped
+        cudaEvent_t b = take_event(h);
+        if (!b) { h->pool.push_back(a); return; }
+        cudaEventRecord(b, h->stream);
+        h->spans.push_back({which, a, b});
     }
 };
 
@@ -253,7 +259,7 @@ void drop_graph(hydro *h)
 int enqueue_device_steps(hydro *h, long long n)
 {
     int rc;
-    const bool use_graph = h->stream != nullptr && !h->profiling && !getenv("HYDRO_NO_GRAPH");
+    const bool use_graph = h->stream != nullptr && !h->profiling && h->graph_replay;
     if (use_graph && !h->step_graph) {
         const long long before = g_launches.load();
         cudaGraph_t graph = nullptr;
@@ -445,15 +451,44 @@ int hydro_set_kernel_variant(hydro_t *h, int variant)
     return HYDRO_OK;
 }
 
+int hydro_set_graph_replay(hydro_t *h, int enable)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "set_graph_replay: NULL handle%s%s");
+    h->graph_replay = enable != 0;
+    if (!h->graph_replay) { CUDA_TRY(cudaStreamSynchronize(h->stream)); drop_graph(h); }
+    return HYDRO_OK;
+}
+
+int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "set_tiling: NULL handle%s%s");
+    if ((tile_rows != 0 && tile_rows != 8 && tile_rows != 16) || planes_per_chunk < 0)
+        return fail(HYDRO_ERR_ARG, "set_tiling: tile_rows must be 0, 8 or 16 and planes_per_chunk >= 0%s%s");
+    CUDA_TRY(cudaStreamSynchronize(h->stream));
+    drop_graph(h);
+    h->ty_req = tile_rows; h->lz_req = planes_per_chunk;
+    cudaError_t e = plan_stage_fused(h->plan, h->g, h->A, h->B, h->ty_req, h->lz_req);
+    if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "set_tiling: %s%s", cudaGetErrorString(e));
+    return HYDRO_OK;
+}
+
+int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long long *blocks)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "get_tiling: NULL handle%s%s");
+    if (tile_rows) *tile_rows = h->plan.ty;
+    if (planes_per_chunk) *planes_per_chunk = h->plan.lz;
+    if (blocks) *blocks = (long long)h->plan.grid.x * h->plan.grid.y * h->plan.grid.z;
+    return HYDRO_OK;
+}
+
 int hydro_set_state(hydro_t *h, const double *U)
 {
     if (!h || !U) return fail(HYDRO_ERR_ARG, "set_state: NULL argument%s%s");
     int rc = copy_state(h, h->A, const_cast<double *>(U), true);
     if (rc) return rc;
     CUDA_TRY(cudaMemsetAsync(h->scal, 0, sizeof(StepScalars), h->stream));
-    bool dev;
-    is_device_pointer(U, &dev);
-    if (!dev) CUDA_TRY(cudaStreamSynchronize(h->stream));   // caller may free U on return
+    CUDA_TRY(cudaStreamSynchronize(h->stream));   // host or device pointer: the caller may free or
+                                                  // overwrite U on return (hydro.h)
     h->t = 0.0; h->step = 0; h->have_state = true; h->smax_valid = false; h->t_on_device = false;
     return HYDRO_OK;
 }
@@ -555,6 +590,7 @@ int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
     if (!h->smax_valid && (rc = launch_cfl_reduce(h))) return rc;
     if ((rc = begin_run(h, t_final))) return rc;
     long long batch = 4;
+    double t_prev = h->t;
     for (;;) {
         if ((rc = enqueue_device_steps(h, batch))) return rc;
         CUDA_TRY(cudaMemcpyAsync(h->scal_host, h->scal, sizeof(StepScalars), cudaMemcpyDeviceToHost,
@@ -566,6 +602,13 @@ int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
             return fail(HYDRO_ERR_UNPHYSICAL, "unphysical state (rho<=0, p<=0 or non-finite speed)%s%s");
         }
         if (sc.done) break;
+        // no progress (dt underflowed to 0, or the signal speed is so large that t + dt == t):
+        // bail out instead of looping forever
+        if (!(sc.dt > 0.0) || !(sc.t > t_prev)) {
+            h->t = sc.t; h->step += sc.steps; h->t_on_device = false;
+            return fail(HYDRO_ERR_UNPHYSICAL, "evolve: the time step no longer advances the clock%s%s");
+        }
+        t_prev = sc.t;
         // size the next batch from the time left and the last dt (wasted identity steps are cheap
         // but not free); never more than 64 steps between host checks
         const double left = (t_final - sc.t) / (sc.dt > 0.0 ? sc.dt : 1.0);

@@ -45,7 +45,10 @@ inline int fused_choose_lz(const Grid &g, int ty, int nsm, int per_sm)
     return best;
 }
 
-inline cudaError_t plan_stage_fused(FusedPlan &p, const Grid &g, const double *A, const double *B)
+// ty_req / lz_req: 0 = choose (hydro_set_tiling); otherwise the tile height (8 | 16) and the planes
+// per z-chunk the caller asked for.
+inline cudaError_t plan_stage_fused(FusedPlan &p, const Grid &g, const double *A, const double *B,
+                                    int ty_req = 0, int lz_req = 0)
 {
     cudaError_t e;
     if ((e = fused_set_attr<1, 16, 1>()) != cudaSuccess) return e;
@@ -55,15 +58,13 @@ inline cudaError_t plan_stage_fused(FusedPlan &p, const Grid &g, const double *A
     int nsm = 148, dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess)
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    // tuning knobs (measurement only): HYDRO_FUSED_TY = 8 | 16, HYDRO_FUSED_LZ = planes per chunk
-    const char *ety = getenv("HYDRO_FUSED_TY"), *elz = getenv("HYDRO_FUSED_LZ");
     // 32 x 16 tiles (one 512-thread block per SM) carry half the per-warp halo / edge work of 32 x 8
     // tiles (two 256-thread blocks per SM) and win on large grids (256^3: 1.615 vs 1.636 ms per
     // step); small grids need the finer tiling to fill the machine
     int ty = g.ny >= 128 ? 16 : 8;
-    if (ety) ty = atoi(ety) == 16 ? 16 : 8;
+    if (ty_req) ty = ty_req == 16 ? 16 : 8;
     int lz = fused_choose_lz(g, ty, nsm, ty == 16 ? 1 : 2);
-    if (elz && atoi(elz) > 0) lz = atoi(elz);
+    if (lz_req > 0) lz = lz_req;
     fused_geometry(p, g, ty, lz);
     p.base[0] = A; p.base[1] = B;
     for (int b = 0; b < 2; ++b)
