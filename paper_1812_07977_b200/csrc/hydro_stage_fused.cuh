@@ -55,7 +55,8 @@ template <int TY> struct FusedSmem {
     static constexpr int OFF_FY = OFF_OY;              //   overwritten in place by the flux through j-1/2
     static constexpr int OFF_IXE = OFF_OY + NVAR * YSZ; // inner x-face value of cell i0+TX, per row
     static constexpr int OFF_IYE = OFF_IXE + NVAR * TY; // inner y-face value of row j0+TY, per col
-    static constexpr int OFF_BAR = OFF_IYE + NVAR * FTX; // FNS TMA mbarriers + 3 phase mbarriers
+    static constexpr int OFF_OXE = OFF_IYE + NVAR * FTX; // outer x-face value of cell i0+TX-1, per row, x2 (plane parity)
+    static constexpr int OFF_BAR = OFF_OXE + 2 * NVAR * TY; // FNS TMA mbarriers + 3 phase mbarriers
     static constexpr int TOTAL = OFF_BAR + FNS + 3 + 1;
     static constexpr size_t BYTES = (size_t)TOTAL * sizeof(double);
     static constexpr unsigned STAGE_BYTES = STAGE * sizeof(double);

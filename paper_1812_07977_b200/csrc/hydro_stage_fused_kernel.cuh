@@ -1,6 +1,9 @@
 // hydro_stage_fused_kernel.cuh -- body of the fused stage kernel (see hydro_stage_fused.cuh).
 #pragma once
-#include <cstdlib>
+
+#ifndef HYD_XFILL
+#define HYD_XFILL 0
+#endif
 
 namespace hyd {
 
@@ -138,6 +141,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         tma::mbar_wait(barW, par);
         // ---- P2: x and y slopes of the own cell (W(k) = Wa), outer face values out ----------
         double Ix[5], Iy[5];
+#if !HYD_XFILL
         {
             double Wm[5], Wp[5], Ox[5];
 #pragma unroll
@@ -146,6 +150,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) Oxs[v * S::XSZ + ty * XP + tx + 1] = Ox[v];
         }
+#endif
         {
             double Wm[5], Wp[5], Oy[5];
 #pragma unroll
@@ -155,7 +160,13 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             for (int v = 0; v < 5; ++v) Oys[v * S::YSZ + (ty + 1) * TX + tx] = Oy[v];
         }
         // halo-cell slopes: x: cells (-1, j) -> outer, (TX, j) -> inner; y: rows -1 -> outer, TY -> inner
-        if (role == 2 || role == 3 || (role == 6 && tx < 2 * TY)) {
+        // (HYD_XFILL: the own x-slopes run after arrive_O, so role 7 also forms the outer value of
+        // cell TX-1 of every row, which the high-edge x-faces of role 0 read right after wait_O)
+        if (role == 2 || role == 3 || (role == 6 && tx < 2 * TY)
+#if HYD_XFILL
+            || (role == 7 && tx < TY)
+#endif
+           ) {
             int cc, st, dst, dstride;
             bool want_outer;
             if (role == 6) {
@@ -163,6 +174,11 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
                 cc = (j + 2) * WP + (hi ? TX + 2 : 1); st = 1; want_outer = !hi;
                 dst = hi ? S::OFF_IXE + j : S::OFF_OX + j * XP;
                 dstride = hi ? TY : S::XSZ;
+#if HYD_XFILL
+            } else if (role == 7) {
+                cc = (tx + 2) * WP + TX + 1; st = 1; want_outer = true;
+                dst = S::OFF_OXE + (c & 1) * NVAR * TY + tx; dstride = TY;
+#endif
             } else {
                 const int hi = role - 2, i = tx;
                 cc = (hi ? TY + 2 : 1) * WP + i + 2; st = WP; want_outer = !hi;
@@ -180,6 +196,18 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         }
         __syncwarp();
         if (tx == 0) tma::mbar_arrive(barO);
+#if HYD_XFILL
+        {   // own x-slopes as filler: the outer values stay inside the warp (lane i -> lane i+1)
+            double Wm[5], Wp[5], Ox[5];
+#pragma unroll
+            for (int v = 0; v < 5; ++v) { Wm[v] = Wsm[v * S::WSZ + wc - 1]; Wp[v] = Wsm[v * S::WSZ + wc + 1]; }
+            HYD_LIMITED_FACES(theta, Wm, Wa, Wp, Ix, Ox);
+            if (tx != TX - 1) {
+#pragma unroll
+                for (int v = 0; v < 5; ++v) Oxs[v * S::XSZ + ty * XP + tx + 1] = Ox[v];
+            }
+        }
+#endif
         // ---- filler O: primitives of raw plane c+4, z-slope of cell plane c+1 ---------------
         double Wn[5], Iz[5], Ozn[5];
         {
@@ -192,6 +220,9 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
         tma::mbar_wait(barO, par);
+#if HYD_XFILL
+        __syncwarp();
+#endif
         // every warp is past P4 of cell plane c-1: raw plane c+1 is dead, refill its stage
         if (t == 0 && c + 5 < nplanes) { tma::fence_proxy_async(); request_plane(c + 5); }
         // ---- P3: x and y fluxes through the low faces ---------------------------------------
@@ -217,7 +248,11 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         if (role == 0 && tx < TY) {
             double L[5], R[5], F[5];
 #pragma unroll
+#if HYD_XFILL
+            for (int v = 0; v < 5; ++v) { L[v] = sm[S::OFF_OXE + (c & 1) * NVAR * TY + v * TY + tx]; R[v] = Ixe[v * TY + tx]; }
+#else
             for (int v = 0; v < 5; ++v) { L[v] = Oxs[v * S::XSZ + tx * XP + TX]; R[v] = Ixe[v * TY + tx]; }
+#endif
             face_flux<0>(L, R, gamma, igm1, F);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Fxs[v * S::XSZ + tx * XP + TX] = F[v];
