@@ -28,6 +28,18 @@
  * P4 bitwise cubic-group symmetry, P5 hand-expanded single-cell update, P6 limiter special
  * cases, P7 HLL closed forms, P8 bitwise translation invariance, P9 wall = mirror,
  * P10 axis relabelling, P11 first dt of config 0.  No function here is "parity unpinned".
+ *
+ * 1D / 2D runs and non-cubic cells (the
+ * RiemannProblem is "an extension of the classic 1D Sod shock tube ... to 2D and 3D"), readings
+ * R21-R24 of DESIGN.md: a run of dimension ndim has its first ndim axes active; an inactive
+ * axis has one cell, no ghost layers, no ghost exchange and no differences, reconstruction or
+ * fluxes (all five variables are still carried); cell edges (dx,dy,dz); the update is
+ * -(dt/dx) * [dFx (+ (dx/dy) dFy (+ (dx/dz) dFz))] and the time step (CFL/ndim) * min_d(dx_d) /
+ * max(|v|+c_s).  With ndim = 3 and dx = dy = dz every operation reduces to the one above bit for
+ * bit (dx/dy = 1 exactly).  Pins: N1 digests of the 3D path before the extension, N2 true-1D Sod
+ * L1 convergence, N3 2D x<->y symmetry bitwise, N4 2D = 3D run of z-uniform data at equal dt,
+ * N5 1D = 2D run of y-uniform data, N6 anisotropic cells: hand-expanded cell update and
+ * relabelling of unequal axes, N7 dt formula values (tests/test_oracle_nd.py).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -42,10 +54,13 @@ enum { NVAR = 5, NG = 2 };
 /* conserved columns: 0 rho, 1 m_x, 2 m_y, 3 m_z, 4 E ; primitive: 0 rho, 1..3 v, 4 p */
 
 typedef struct oracle_hydro {
-    int nx, ny, nz;           /* active cells */
-    int Nx, Ny, Nz;           /* padded = active + 2*NG */
+    int ndim;                 /* active axes: x (1), x,y (2), x,y,z (3) */
+    int nx, ny, nz;           /* active cells (1 on an inactive axis) */
+    int gx, gy, gz;           /* ghost layers per side: NG on an active axis, 0 otherwise */
+    int Nx, Ny, Nz;           /* padded = active + 2*ghost */
     long ncell;               /* padded cells per column */
     double gamma, gm1, igm1, theta, dx, cfl;
+    double dxyz[3];           /* cell edges; dx == dxyz[0] */
     int bc[6];                /* xlo,xhi,ylo,yhi,zlo,zhi */
     double t;
     long long step;
@@ -134,23 +149,32 @@ void oracle_hll_flux(double gamma, int d, const double WL[5], const double WR[5]
 
 /* ------------------------------------------------------------------ handle */
 
-int oracle_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6],
-                  oracle_hydro_t **out)
+/* Initialize for a run of dimension ndim (R21): n[a] >= 2 and d[a] > 0 on the
+ * active axes a < ndim, n[a] == 1 on the others (their d[a] and bc entries are ignored). */
+int oracle_create_nd(int ndim, const int n[3], const double d[3], double gamma, const int bc[6],
+                     oracle_hydro_t **out)
 {
-    if (!out || !bc) return ERR_ARG;
+    if (!out || !bc || !n || !d) return ERR_ARG;
     *out = NULL;
-    if (nx < 2 || ny < 2 || nz < 2 || !(gamma > 1.0) || !(dx > 0.0) || !isfinite(dx) ||
-        !isfinite(gamma)) return ERR_ARG;
-    for (int f = 0; f < 6; ++f) if (bc[f] < 0 || bc[f] > 2) return ERR_ARG;
-    for (int a = 0; a < 3; ++a)
-        if ((bc[2 * a] == BC_PERIODIC) != (bc[2 * a + 1] == BC_PERIODIC)) return ERR_ARG;
+    if (ndim < 1 || ndim > 3 || !(gamma > 1.0) || !isfinite(gamma)) return ERR_ARG;
+    for (int a = 0; a < 3; ++a) {
+        if (a < ndim) {
+            if (n[a] < 2 || !(d[a] > 0.0) || !isfinite(d[a])) return ERR_ARG;
+            if (bc[2 * a] < 0 || bc[2 * a] > 2 || bc[2 * a + 1] < 0 || bc[2 * a + 1] > 2) return ERR_ARG;
+            if ((bc[2 * a] == BC_PERIODIC) != (bc[2 * a + 1] == BC_PERIODIC)) return ERR_ARG;
+        } else if (n[a] != 1) return ERR_ARG;
+    }
     oracle_hydro_t *h = (oracle_hydro_t *)calloc(1, sizeof *h);
     if (!h) return ERR_ALLOC;
-    h->nx = nx; h->ny = ny; h->nz = nz;
-    h->Nx = nx + 2 * NG; h->Ny = ny + 2 * NG; h->Nz = nz + 2 * NG;
+    h->ndim = ndim;
+    h->nx = n[0]; h->ny = n[1]; h->nz = n[2];
+    h->gx = NG; h->gy = ndim >= 2 ? NG : 0; h->gz = ndim >= 3 ? NG : 0;
+    h->Nx = h->nx + 2 * h->gx; h->Ny = h->ny + 2 * h->gy; h->Nz = h->nz + 2 * h->gz;
     h->ncell = (long)h->Nx * h->Ny * h->Nz;
     h->gamma = gamma; h->gm1 = gamma - 1.0; h->igm1 = 1.0 / h->gm1;
-    h->theta = 1.4; h->dx = dx; h->cfl = 0.7;
+    h->theta = 1.4; h->cfl = 0.7;
+    for (int a = 0; a < 3; ++a) h->dxyz[a] = a < ndim ? d[a] : d[0];
+    h->dx = d[0];
     memcpy(h->bc, bc, sizeof h->bc);
     size_t col = (size_t)h->ncell * sizeof(double);
     double **blocks[] = { &h->FluidCurrent, &h->FluidOld, &h->Primitive, &h->Differences,
@@ -168,6 +192,17 @@ fail:
     free(h->ReconInner); free(h->ReconOuter); free(h->Fluxes); free(h->FluidUpdate);
     free(h->FluxDifference); free(h);
     return ERR_ALLOC;
+}
+
+/* The 3D run with cubic cells of edge dx (R13). */
+int oracle_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6],
+                  oracle_hydro_t **out)
+{
+    const int n[3] = { nx, ny, nz };
+    const double d[3] = { dx, dx, dx };
+    if (out) *out = NULL;
+    if (nx < 2 || ny < 2 || nz < 2) return ERR_ARG;
+    return oracle_create_nd(3, n, d, gamma, bc, out);
 }
 
 int oracle_destroy(oracle_hydro_t *h)
@@ -232,7 +267,7 @@ int oracle_set_state(oracle_hydro_t *h, const double *U)
         for (int k = 0; k < h->nz; ++k)
             for (int j = 0; j < h->ny; ++j)
                 for (int i = 0; i < h->nx; ++i)
-                    col[IDX(h, i + NG, j + NG, k + NG)] =
+                    col[IDX(h, i + h->gx, j + h->gy, k + h->gz)] =
                         U[v * nact + ((long)k * h->ny + j) * h->nx + i];
     }
     h->t = 0.0; h->step = 0; h->have_state = 1;
@@ -250,7 +285,7 @@ int oracle_get_state(oracle_hydro_t *h, double *U)
             for (int j = 0; j < h->ny; ++j)
                 for (int i = 0; i < h->nx; ++i)
                     U[v * nact + ((long)k * h->ny + j) * h->nx + i] =
-                        col[IDX(h, i + NG, j + NG, k + NG)];
+                        col[IDX(h, i + h->gx, j + h->gy, k + h->gz)];
     }
     return OK;
 }
@@ -271,14 +306,15 @@ int oracle_get_padded(oracle_hydro_t *h, double *Upad)
 static void ghost_axis(oracle_hydro_t *h, double *Value, int a)
 {
     const int n[3] = { h->nx, h->ny, h->nz };
+    const int g[3] = { h->gx, h->gy, h->gz };
     const long s[3] = { 1, h->Nx, (long)h->Nx * h->Ny };
     const int t1 = (a + 1) % 3, t2 = (a + 2) % 3;
     const int na = n[a];
     for (int v = 0; v < NVAR; ++v) {
         double *col = Value + v * h->ncell;
         const double sgn = (v == 1 + a) ? -1.0 : 1.0;   /* normal momentum flips at a wall */
-        for (int q2 = NG; q2 < n[t2] + NG; ++q2)
-            for (int q1 = NG; q1 < n[t1] + NG; ++q1) {
+        for (int q2 = g[t2]; q2 < n[t2] + g[t2]; ++q2)
+            for (int q1 = g[t1]; q1 < n[t1] + g[t1]; ++q1) {
                 double *row = col + q1 * s[t1] + q2 * s[t2];
 #define A(I) row[(long)(I) * s[a]]
                 switch (h->bc[2 * a]) {              /* low side: ghosts 0,1 */
@@ -298,7 +334,7 @@ static void ghost_axis(oracle_hydro_t *h, double *Value, int a)
 
 static void GhostExchange(oracle_hydro_t *h, double *Value)
 {
-    for (int a = 0; a < 3; ++a) ghost_axis(h, Value, a);
+    for (int a = 0; a < h->ndim; ++a) ghost_axis(h, Value, a);      /* active axes only (R21) */
 }
 
 /* Test hook: run GhostExchange on FluidCurrent. */
@@ -322,9 +358,9 @@ static void ComputePrimitive(oracle_hydro_t *h, const double *Value)
 #pragma omp parallel for collapse(2) schedule(static)
     for (int K = 0; K < h->Nz; ++K)
         for (int J = 0; J < h->Ny; ++J) {
-            int gK = (K < NG || K >= h->nz + NG), gJ = (J < NG || J >= h->ny + NG);
+            int gK = (K < h->gz || K >= h->nz + h->gz), gJ = (J < h->gy || J >= h->ny + h->gy);
             for (int I = 0; I < h->Nx; ++I) {
-                int gI = (I < NG || I >= h->nx + NG);
+                int gI = (I < h->gx || I >= h->nx + h->gx);
                 if (gK + gJ + gI > 1) continue;            /* edge / corner: never read */
                 long c = IDX(h, I, J, K);
                 double U[5], W[5];
@@ -339,8 +375,8 @@ static void ComputePrimitive(oracle_hydro_t *h, const double *Value)
  * lo..hi (inclusive); the other two axes run over active cells only. */
 #define DIM_LOOP_BEGIN(h, d, lo, hi)                                                   \
     {                                                                                  \
-        int lo_[3] = { NG, NG, NG };                                                   \
-        int hi_[3] = { (h)->nx + NG - 1, (h)->ny + NG - 1, (h)->nz + NG - 1 };         \
+        int lo_[3] = { (h)->gx, (h)->gy, (h)->gz };                                    \
+        int hi_[3] = { (h)->nx + (h)->gx - 1, (h)->ny + (h)->gy - 1, (h)->nz + (h)->gz - 1 }; \
         lo_[d] = (lo); hi_[d] = (hi);                                                  \
         _Pragma("omp parallel for collapse(2) schedule(static)")                       \
         for (int K = lo_[2]; K <= hi_[2]; ++K)                                         \
@@ -425,17 +461,28 @@ static void ComputeFluxDifference(oracle_hydro_t *h, int d)
     DIM_LOOP_END
 }
 
-/* ComputeUpdate(TimeStep) -> FluidUpdate (O5): -(dt/dx) * sum3 of the three
- * per-dimension flux differences. */
+/* ComputeUpdate(TimeStep) -> FluidUpdate (O5 / R23): -(dt/dx) times the sum over
+ * the active dimensions of the flux differences, those of y and z scaled by dx/dy and dx/dz
+ * (exactly 1 for cubic cells).  Three dimensions: sum3; two: a plain sum; one: the x term. */
 static void ComputeUpdate(oracle_hydro_t *h, double dt)
 {
     const long nc = h->ncell;
     const double r = dt / h->dx;
+    const double ry = h->dx / h->dxyz[1], rz = h->dx / h->dxyz[2];
+    const int ndim = h->ndim;
     const double *dFx = h->FluxDifference, *dFy = dFx + NVAR * nc, *dFz = dFy + NVAR * nc;
     double *dU = h->FluidUpdate;
     DIM_LOOP_BEGIN(h, 0, NG, h->nx + NG - 1)
         for (int v = 0; v < NVAR; ++v) {
-            double D = oracle_sum3(dFx[v * nc + c], dFy[v * nc + c], dFz[v * nc + c]);
+            double D = dFx[v * nc + c];
+            if (ndim == 2) {
+                double ty = ry * dFy[v * nc + c];
+                D = D + ty;
+            } else if (ndim == 3) {
+                double ty = ry * dFy[v * nc + c];
+                double tz = rz * dFz[v * nc + c];
+                D = oracle_sum3(D, ty, tz);
+            }
             dU[v * nc + c] = -(r * D);
         }
     DIM_LOOP_END
@@ -446,7 +493,7 @@ static void ComputeUpdate(oracle_hydro_t *h, double dt)
 static void Substep(oracle_hydro_t *h, double dt)
 {
     ComputePrimitive(h, h->FluidCurrent);
-    for (int d = 0; d < 3; ++d) {
+    for (int d = 0; d < h->ndim; ++d) {
         ComputeDifferences(h, d);
         ComputeReconstruction(h, d);
         ComputeFluxes(h, d);
@@ -499,9 +546,9 @@ int oracle_max_signal_speed(oracle_hydro_t *h, double *smax_out)
     double smax = 0.0;
     int bad = 0;
 #pragma omp parallel for collapse(2) schedule(static) reduction(max : smax) reduction(| : bad)
-    for (int K = NG; K < h->nz + NG; ++K)
-        for (int J = NG; J < h->ny + NG; ++J)
-            for (int I = NG; I < h->nx + NG; ++I) {
+    for (int K = h->gz; K < h->nz + h->gz; ++K)
+        for (int J = h->gy; J < h->ny + h->gy; ++J)
+            for (int I = h->gx; I < h->nx + h->gx; ++I) {
                 long c = IDX(h, I, J, K);
                 double rho = Cur[c], mx = Cur[nc + c], my = Cur[2 * nc + c],
                        mz = Cur[3 * nc + c], E = Cur[4 * nc + c];
@@ -522,15 +569,18 @@ int oracle_max_signal_speed(oracle_hydro_t *h, double *smax_out)
     return bad ? ERR_UNPHYSICAL : OK;
 }
 
-/* dt = (CFL/3) * (dx / smax)   (R8: Courant factor divided by the 3 unsplit dimensions). */
+/* dt = (CFL/ndim) * (min_d dx_d / smax)   (R8 / R22: Courant factor divided by the number of
+ * unsplit dimensions, smallest edge of the cell). */
 int oracle_cfl_dt(oracle_hydro_t *h, double *dt)
 {
     if (!h || !dt) return ERR_ARG;
     double smax;
     int rc = oracle_max_signal_speed(h, &smax);
     if (rc != OK) return rc;
-    double c3 = h->cfl / 3.0;
-    double dxs = h->dx / smax;
+    double dmin_ = h->dxyz[0];
+    for (int a = 1; a < h->ndim; ++a) dmin_ = dmin(dmin_, h->dxyz[a]);
+    double c3 = h->cfl / (double)h->ndim;
+    double dxs = dmin_ / smax;
     *dt = c3 * dxs;
     return OK;
 }

@@ -44,6 +44,8 @@ def lib():
         vp = C.c_void_p
         L.oracle_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                                     C.POINTER(C.c_int), C.POINTER(vp)]
+        L.oracle_create_nd.argtypes = [C.c_int, C.POINTER(C.c_int), _dp, C.c_double,
+                                       C.POINTER(C.c_int), C.POINTER(vp)]
         L.oracle_destroy.argtypes = [vp]
         L.oracle_set_state.argtypes = [vp, _dp]
         L.oracle_get_state.argtypes = [vp, _dp]
@@ -110,12 +112,21 @@ def get_threads():
 class OracleHydro:
     """Same call names as the C-ABI of the product (``include/hydro.h``), oracle side."""
 
-    def __init__(self, nx, ny, nz, gamma, dx, bc):
+    def __init__(self, nx, ny, nz, gamma, dx, bc, ndim=None, dxyz=None):
+        """3D run with cubic cells (oracle_create) or, with `ndim` given, a run of dimension ndim
+        with cell edges `dxyz` (oracle_create_nd; extents of inactive axes must be 1)."""
         self.shape = (5, nz, ny, nx)
-        self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
         self._h = C.c_void_p()
         arr = (C.c_int * 6)(*[int(b) for b in bc])
-        self._chk(lib().oracle_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "create")
+        if ndim is None:
+            self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
+            self._chk(lib().oracle_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "create")
+        else:
+            g = [4 if a < ndim else 0 for a in range(3)]
+            self.padded_shape = (5, nz + g[2], ny + g[1], nx + g[0])
+            n = (C.c_int * 3)(nx, ny, nz)
+            d = (C.c_double * 3)(*(dxyz if dxyz is not None else (dx, dx, dx)))
+            self._chk(lib().oracle_create_nd(ndim, n, d, gamma, arr, C.byref(self._h)), "create_nd")
 
     @staticmethod
     def _chk(rc, where):
