@@ -62,25 +62,18 @@ __device__ __forceinline__ void prim5(const double U[5], double gm1, double W[5]
     W[4] = gm1 * fma(-0.5 * U[0], q, U[4]);
 }
 
-// O3: limited slope of one cell; hs = 0.5 * sigma is formed directly:
-//   0.5*min(theta|a|, theta|b|, 0.5|a+b|) = min((0.5 theta) min(|a|,|b|), 0.25|a+b|)
-// (exactly, scaling by powers of two and monotone rounding), sign of a when a and b agree in
-// sign, else zero -- decided on the sign bits.
-#ifndef HYD_LIM
-#define HYD_LIM 0
-#endif
-#ifndef HYD_HLLMAX
-#define HYD_HLLMAX 0
-#endif
+// O3: limited slope of one cell, hs = 0.5 * sigma, in a select-free form on the fp64 pipe (the
+// kernel is limited by issue slots as much as by the pipe; the comparison form costs 11 integer /
+// select instructions per slope, this one a single LOP3).  With c = a + b and d = a - b:
+//   g = |c| - |d| = +2 min(|a|,|b|) when a and b agree in sign, -2 min(|a|,|b|) otherwise;
+//   R = 2 min(theta g, |c|)  through  min(x,y) = (x + y - |x - y|)/2;
+//   T = R + |R| = 2 max(0, R) = 8 min(theta|a|, theta|b|, |a+b|/2)  or 0;   hs = T/16, sign of c.
+// Exact where it matters (a = b = 0 gives 0; opposite signs give exactly 0); elsewhere within a
+// few ulp of the jump |c| of the comparison form (R20).
 __device__ __forceinline__ void limited_faces(double half_theta, const double Wm[5],
                                               const double Wc[5], const double Wp[5],
                                               double inner[5], double outer[5])
 {
-#if HYD_LIM == 1
-    // select-free form on the fp64 pipe: with c = a + b and d = a - b,
-    //   g = |c| - |d| = +2 min(|a|,|b|) when a and b agree in sign, -2 min(|a|,|b|) otherwise;
-    //   R = 2 min(theta g, |c|) via min(x,y) = (x + y - |x - y|)/2;  T = R + |R| = 2 max(0, R);
-    //   hs = T/16 with the sign of c.
     const double th = 2.0 * half_theta;
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
@@ -95,23 +88,6 @@ __device__ __forceinline__ void limited_faces(double half_theta, const double Wm
         inner[v] = fma(-0.0625, Ts, Wc[v]);
         outer[v] = fma(0.0625, Ts, Wc[v]);
     }
-#else
-#pragma unroll
-    for (int v = 0; v < 5; ++v) {
-        const double a = Wc[v] - Wm[v];
-        const double b = Wp[v] - Wc[v];
-        const double mn = fabs(a) < fabs(b) ? a : b;      // one DSETP; the integer form costs more issue slots
-        const double t1 = half_theta * fabs(mn);
-        const double t2 = 0.25 * fabs(a + b);
-        const double h = min_nonneg(t1, t2);
-        const int ah = __double2hiint(a), bh = __double2hiint(b);
-        const bool same = (ah ^ bh) >= 0;
-        const int hh = __double2hiint(h) | (ah & 0x80000000);
-        const double hs = __hiloint2double(same ? hh : 0, same ? __double2loint(h) : 0);
-        inner[v] = Wc[v] - hs;
-        outer[v] = Wc[v] + hs;
-    }
-#endif
 }
 
 // O4: HLL flux, components in (rho, n, t1, t2, E) order; inputs (rho, vn, vt1, vt2, p).
@@ -137,22 +113,8 @@ __device__ __forceinline__ void hll_flux(const double L[5], const double R[5], d
         FR[0] = UR[1]; FR[1] = fma(UR[1], R[1], R[4]); FR[2] = UR[2] * R[1]; FR[3] = UR[3] * R[1];
         FR[4] = (E + R[4]) * R[1];
     }
-#if HYD_HLLMAX == 1
-    // max(x, y) = (x + y + |x - y|)/2 and max(0, z) = (z + |z|)/2 on the fp64 pipe (no selects):
-    // ap4 = 4 max(0, x, y)
-    double ap, am;
-    {
-        const double x = L[1] + cL, y = R[1] + cR;
-        const double m2 = (x + y) + fabs(x - y);
-        ap = 0.25 * (m2 + fabs(m2));
-        const double xm = cL - L[1], ym = cR - R[1];
-        const double n2 = (xm + ym) + fabs(xm - ym);
-        am = 0.25 * (n2 + fabs(n2));
-    }
-#else
     const double ap = dmax(0.0, dmax(L[1] + cL, R[1] + cR));
     const double am = dmax(0.0, dmax(cL - L[1], cR - R[1]));
-#endif
     const double w = rcp(ap + am);
     const double al = ap * w, be = am * w, de = (ap * am) * w;
 #pragma unroll

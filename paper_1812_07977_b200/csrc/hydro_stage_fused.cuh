@@ -49,7 +49,8 @@ template <int TY> struct FusedSmem {
     static constexpr int YSZ = (TY + 1) * FTX;
     static constexpr int OFF_RING = 0;                 // raw conserved planes, filled by TMA
     static constexpr int OFF_W = OFF_RING + FNS * STAGE;  // primitives of the plane being updated
-    static constexpr int OFF_OX = OFF_W + STAGE;       // outer x-face value of cell i-1 at slot i;
+    static constexpr int NW = TY == 16 ? 2 : 1;        // primitive tiles (2: by plane parity, no W barrier)
+    static constexpr int OFF_OX = OFF_W + NW * STAGE;  // outer x-face value of cell i-1 at slot i;
     static constexpr int OFF_FX = OFF_OX;              //   overwritten in place by the flux through i-1/2
     static constexpr int OFF_OY = OFF_OX + NVAR * XSZ; // outer y-face value of row j-1 at row j;
     static constexpr int OFF_FY = OFF_OY;              //   overwritten in place by the flux through j-1/2

@@ -1,10 +1,6 @@
 // hydro_stage_fused_kernel.cuh -- body of the fused stage kernel (see hydro_stage_fused.cuh).
 #pragma once
 
-#ifndef HYD_XFILL
-#define HYD_XFILL 0
-#endif
-
 namespace hyd {
 
 struct FusedArgs {
@@ -20,12 +16,18 @@ struct FusedArgs {
 
 // `umap` describes the stencil input (stage 1: U0, stage 2: U1; ghost-filled) to the TMA unit.
 //
-// Synchronisation.  The x/y exchange of one plane needs three block-wide hand-offs (primitives,
-// outer face values, fluxes).  Each is a split-phase mbarrier: a warp ARRIVES as soon as its
-// stores are done, then does z-direction work that needs no one else (the filler), and only then
-// WAITS.  The skew between warps is absorbed by the fillers instead of idling at a barrier.
-//   per cell plane c:  wait_W  P2  arrive_O  [prim(c+4), z-slope]  wait_O  P3  arrive_F
-//                      [z-flux, primitive tile of plane c+1, arrive_W(c+1)]  wait_F  P4
+// Synchronisation.  The x/y exchange of one plane needs block-wide hand-offs (primitives, outer
+// face values, fluxes).  Each is a split-phase mbarrier: a warp ARRIVES as soon as its stores are
+// done, then does work that needs no other warp (the filler), and only then WAITS.  The skew
+// between warps is absorbed by the fillers instead of idling at a barrier.
+//   TY = 16 (PIPE): the primitive tile is double-buffered by plane parity, so its hand-off rides on
+//   the flux barrier, and only the y-slopes (and the halo-cell slopes) precede the face-value
+//   barrier -- the x-slopes stay inside the warp (lane i -> lane i+1) and run as filler:
+//     per cell plane c:  y-slopes, halo slopes  arrive_O  [x-slopes, prim(c+4), z-slope]  wait_O
+//                        tile(c+1), x/y fluxes, edge fluxes  arrive_F  [z-flux]  wait_F  update
+//   TY = 8 (two blocks per SM, single primitive tile):
+//     per cell plane c:  wait_W  x/y slopes  arrive_O  [prim(c+4), z-slope]  wait_O  fluxes  arrive_F
+//                        [z-flux, tile(c+1), arrive_W(c+1)]  wait_F  update
 template <int STAGE, int TY, int MINB>
 __global__ void __launch_bounds__(FTX * TY, MINB)
 stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
@@ -33,7 +35,8 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     using S = FusedSmem<TY>;
     constexpr int TX = FTX, WP = S::WP, XP = S::XP;
     extern __shared__ __align__(128) double sm[];
-    double *Wsm = sm + S::OFF_W, *Oxs = sm + S::OFF_OX, *Oys = sm + S::OFF_OY;
+    constexpr bool PIPE = S::NW == 2;      // see "Synchronisation" above
+    double *Oxs = sm + S::OFF_OX, *Oys = sm + S::OFF_OY;
     double *Fxs = sm + S::OFF_FX, *Fys = sm + S::OFF_FY;
     double *Ixe = sm + S::OFF_IXE, *Iye = sm + S::OFF_IYE;
     uint64_t *bar = reinterpret_cast<uint64_t *>(sm + S::OFF_BAR);     // TMA: plane p -> bar[p % FNS]
@@ -81,7 +84,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const double r = a.dev_dt ? a.dev_dt->dt / a.dx : a.dt_over_dx;
 
     // primitive tile of one cell plane: own cell from registers, halo cells from the raw plane
-    auto write_tile = [&](const double Wown[5], const double *Uraw, int role) {
+    auto write_tile = [&](double *Wsm, const double Wown[5], const double *Uraw, int role) {
 #pragma unroll
         for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + wc] = Wown[v];
         const int th = (role - 3) * TX + tx;                  // halo cell index -> plane coords (hc, hr)
@@ -97,8 +100,10 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + hw] = Wh[v];
         }
-        __syncwarp();
-        if (tx == 0) tma::mbar_arrive(barW);
+        if (!PIPE) {
+            __syncwarp();
+            if (tx == 0) tma::mbar_arrive(barW);
+        }
     };
 
     // ---- prologue: raw planes 0..3 -> W(k0), W(k0+1), outer_z(k0), flux through face k0-1/2 ----
@@ -130,7 +135,8 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             if (t == 0) { tma::fence_proxy_async(); request_plane(4); }
         }
     }
-    write_tile(Wa, sm + S::OFF_RING + 2 * S::STAGE, ty);      // cell plane 0 = raw plane 2; arrive_W(0)
+    write_tile(sm + S::OFF_W, Wa, sm + S::OFF_RING + 2 * S::STAGE, ty);   // cell plane 0 = raw plane 2; arrive_W(0)
+    if (PIPE) __syncthreads();
 
 #pragma unroll 1
     for (int c = 0; c < nc; ++c) {
@@ -138,11 +144,11 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         const int role = (ty + c) & (TY - 1);
         const double *Uk = sm + S::OFF_RING + ((c + 2) % FNS) * S::STAGE;      // raw plane of cell plane c
         const long long cg = col + g.sy * (long long)(k0 + c + NG);
-        tma::mbar_wait(barW, par);
+        double *Wsm = sm + S::OFF_W + (PIPE ? (c & 1) * S::STAGE : 0);
+        if (!PIPE) tma::mbar_wait(barW, par);
         // ---- P2: x and y slopes of the own cell (W(k) = Wa), outer face values out ----------
         double Ix[5], Iy[5];
-#if !HYD_XFILL
-        {
+        if (!PIPE) {
             double Wm[5], Wp[5], Ox[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { Wm[v] = Wsm[v * S::WSZ + wc - 1]; Wp[v] = Wsm[v * S::WSZ + wc + 1]; }
@@ -150,7 +156,6 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) Oxs[v * S::XSZ + ty * XP + tx + 1] = Ox[v];
         }
-#endif
         {
             double Wm[5], Wp[5], Oy[5];
 #pragma unroll
@@ -160,13 +165,9 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             for (int v = 0; v < 5; ++v) Oys[v * S::YSZ + (ty + 1) * TX + tx] = Oy[v];
         }
         // halo-cell slopes: x: cells (-1, j) -> outer, (TX, j) -> inner; y: rows -1 -> outer, TY -> inner
-        // (HYD_XFILL: the own x-slopes run after arrive_O, so role 7 also forms the outer value of
-        // cell TX-1 of every row, which the high-edge x-faces of role 0 read right after wait_O)
-        if (role == 2 || role == 3 || (role == 6 && tx < 2 * TY)
-#if HYD_XFILL
-            || (role == 7 && tx < TY)
-#endif
-           ) {
+        // (PIPE: the own x-slopes run after arrive_O, so role 7 also forms the outer value of cell
+        // TX-1 of every row, which the high-edge x-faces of role 0 read right after wait_O)
+        if (role == 2 || role == 3 || (role == 6 && tx < 2 * TY) || (PIPE && role == 7 && tx < TY)) {
             int cc, st, dst, dstride;
             bool want_outer;
             if (role == 6) {
@@ -174,11 +175,9 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
                 cc = (j + 2) * WP + (hi ? TX + 2 : 1); st = 1; want_outer = !hi;
                 dst = hi ? S::OFF_IXE + j : S::OFF_OX + j * XP;
                 dstride = hi ? TY : S::XSZ;
-#if HYD_XFILL
-            } else if (role == 7) {
+            } else if (PIPE && role == 7) {
                 cc = (tx + 2) * WP + TX + 1; st = 1; want_outer = true;
                 dst = S::OFF_OXE + (c & 1) * NVAR * TY + tx; dstride = TY;
-#endif
             } else {
                 const int hi = role - 2, i = tx;
                 cc = (hi ? TY + 2 : 1) * WP + i + 2; st = WP; want_outer = !hi;
@@ -196,8 +195,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         }
         __syncwarp();
         if (tx == 0) tma::mbar_arrive(barO);
-#if HYD_XFILL
-        {   // own x-slopes as filler: the outer values stay inside the warp (lane i -> lane i+1)
+        if (PIPE) {   // own x-slopes as filler: the outer values stay inside the warp (lane i -> lane i+1)
             double Wm[5], Wp[5], Ox[5];
 #pragma unroll
             for (int v = 0; v < 5; ++v) { Wm[v] = Wsm[v * S::WSZ + wc - 1]; Wp[v] = Wsm[v * S::WSZ + wc + 1]; }
@@ -207,7 +205,6 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
                 for (int v = 0; v < 5; ++v) Oxs[v * S::XSZ + ty * XP + tx + 1] = Ox[v];
             }
         }
-#endif
         // ---- filler O: primitives of raw plane c+4, z-slope of cell plane c+1 ---------------
         double Wn[5], Iz[5], Ozn[5];
         {
@@ -220,13 +217,16 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
         tma::mbar_wait(barO, par);
-#if HYD_XFILL
-        __syncwarp();
-#endif
+        if (PIPE) __syncwarp();                               // the warp's own outer x values are in place
         // every warp is past P4 of cell plane c-1: raw plane c+1 is dead, refill its stage
         if (t == 0 && c + 5 < nplanes) { tma::fence_proxy_async(); request_plane(c + 5); }
         // ---- P3: x and y fluxes through the low faces ---------------------------------------
         double Fxl[5], Fyl[5];
+        // PIPE: primitive tile of cell plane c+1 into the other buffer (free since wait_F(c-1), read
+        // after wait_F(c)); own cell = W(c+1) = Wb, halo cells from raw plane c+3
+        if (PIPE && c + 1 < nc)
+            write_tile(sm + S::OFF_W + ((c + 1) & 1) * S::STAGE, Wb,
+                       sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE, (ty + c + 1) & (TY - 1));
         {
             double L[5];
 #pragma unroll
@@ -247,12 +247,10 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         // column `lane` (each flux is written over the outer value it consumed)
         if (role == 0 && tx < TY) {
             double L[5], R[5], F[5];
+            const double *Le = PIPE ? sm + S::OFF_OXE + (c & 1) * NVAR * TY + tx : Oxs + tx * XP + TX;
+            constexpr int les = PIPE ? TY : S::XSZ;
 #pragma unroll
-#if HYD_XFILL
-            for (int v = 0; v < 5; ++v) { L[v] = sm[S::OFF_OXE + (c & 1) * NVAR * TY + v * TY + tx]; R[v] = Ixe[v * TY + tx]; }
-#else
-            for (int v = 0; v < 5; ++v) { L[v] = Oxs[v * S::XSZ + tx * XP + TX]; R[v] = Ixe[v * TY + tx]; }
-#endif
+            for (int v = 0; v < 5; ++v) { L[v] = Le[v * les]; R[v] = Ixe[v * TY + tx]; }
             face_flux<0>(L, R, gamma, igm1, F);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Fxs[v * S::XSZ + tx * XP + TX] = F[v];
@@ -282,8 +280,8 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
                 dFz[v] = Fzp[v] - Fzm[v]; Fzm[v] = Fzp[v]; Oz[v] = Ozn[v]; Wa[v] = Wb[v]; Wb[v] = Wn[v];
             }
         }
-        if (c + 1 < nc)                                       // arrive_W(c+1)
-            write_tile(Wa, sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE, (ty + c + 1) & (TY - 1));
+        if (!PIPE && c + 1 < nc)                            // arrive_W(c+1)
+            write_tile(Wsm, Wa, sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE, (ty + c + 1) & (TY - 1));
         tma::mbar_wait(barF, par);
         // ---- P4: divergence, RK combine, store, CFL ------------------------------------------
         double un[5];
