@@ -16,17 +16,16 @@
 namespace hyd {
 namespace fast {
 
-// 1/x, x > 0 finite and normal.  Seed has ~20 good bits; two Newton steps (measured on B200:
-// equal to the IEEE quotient on 2^26 arguments; one step leaves 4e3 ulp).
+// 1/x, x > 0 finite and normal.  The MUFU.RCP64H seed is good to ~2^-20; one third-order step
+// y (1 + e + e^2), e = 1 - x y, leaves e^3 ~ 2^-60 plus the rounding of the last fma (<= 1 ulp
+// measured; the previous form, two Newton steps, cost one more DFMA).
 __device__ __forceinline__ double rcp(double x)
 {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    return y;
+    const double e = fma(-x, y, 1.0);
+    const double t = fma(e, e, e);
+    return fma(y, t, y);
 }
 
 // 1/sqrt(x), x > 0 finite and normal.  One third-order step on the ~2^-20 seed: measured on
@@ -52,24 +51,33 @@ __device__ __forceinline__ double max_nonneg(double x, double y)
     return __double_as_longlong(x) > __double_as_longlong(y) ? x : y;
 }
 
+// max(0, x) on the sign bit (integer pipe: one ISETP + two SEL instead of DSETP + two FSEL)
+__device__ __forceinline__ double max0(double x)
+{
+    const int hi = __double2hiint(x);
+    return __hiloint2double(hi < 0 ? 0 : hi, hi < 0 ? 0 : __double2loint(x));
+}
+
 // O2: conserved -> primitive (rho, vx, vy, vz, p)
 __device__ __forceinline__ void prim5(const double U[5], double gm1, double W[5])
 {
     const double inv = rcp(U[0]);
     W[0] = U[0];
     W[1] = U[1] * inv; W[2] = U[2] * inv; W[3] = U[3] * inv;
-    const double q = fma(W[1], W[1], fma(W[2], W[2], W[3] * W[3]));
-    W[4] = gm1 * fma(-0.5 * U[0], q, U[4]);
+    const double rq = fma(U[1], W[1], fma(U[2], W[2], U[3] * W[3]));     // rho |v|^2 = m . v
+    W[4] = gm1 * fma(-0.5, rq, U[4]);
 }
 
 // O3: limited slope of one cell, hs = 0.5 * sigma, in a select-free form on the fp64 pipe (the
 // kernel is limited by issue slots as much as by the pipe; the comparison form costs 11 integer /
-// select instructions per slope, this one a single LOP3).  With c = a + b and d = a - b:
+// select instructions per slope, this one a single LOP3).  With c = a + b = W(+1) - W(-1) and
+// d = a - b:
 //   g = |c| - |d| = +2 min(|a|,|b|) when a and b agree in sign, -2 min(|a|,|b|) otherwise;
-//   R = 2 min(theta g, |c|)  through  min(x,y) = (x + y - |x - y|)/2;
-//   T = R + |R| = 2 max(0, R) = 8 min(theta|a|, theta|b|, |a+b|/2)  or 0;   hs = T/16, sign of c.
+//   T = theta|g| + |c| - |theta g - |c|| = 2 clamp(theta g, 0, |c|)      (clamp(x,0,y) = (|x| + y - |x-y|)/2)
+//     = 4 min(theta|a|, theta|b|, |a+b|/2) when the signs agree, exactly 0 otherwise;
+//   hs = T/8 with the sign of c.
 // Exact where it matters (a = b = 0 gives 0; opposite signs give exactly 0); elsewhere within a
-// few ulp of the jump |c| of the comparison form (R20).
+// few ulp of the jump |c| of the comparison form (R20).  Nine fp64 instructions.
 __device__ __forceinline__ void limited_faces(double half_theta, const double Wm[5],
                                               const double Wc[5], const double Wp[5],
                                               double inner[5], double outer[5])
@@ -80,13 +88,12 @@ __device__ __forceinline__ void limited_faces(double half_theta, const double Wm
         const double c = Wp[v] - Wm[v];
         const double d = fma(2.0, Wc[v], -Wm[v]) - Wp[v];
         const double g = fabs(c) - fabs(d);
-        const double P = fma(th, g, fabs(c));
-        const double Q = fma(th, g, -fabs(c));
-        const double R = P - fabs(Q);
-        const double T = R + fabs(R);
+        const double u = fma(th, g, -fabs(c));
+        const double w = fma(th, fabs(g), fabs(c));
+        const double T = w - fabs(u);
         const double Ts = __hiloint2double(__double2hiint(T) | (__double2hiint(c) & 0x80000000), __double2loint(T));
-        inner[v] = fma(-0.0625, Ts, Wc[v]);
-        outer[v] = fma(0.0625, Ts, Wc[v]);
+        inner[v] = fma(-0.125, Ts, Wc[v]);
+        outer[v] = fma(0.125, Ts, Wc[v]);
     }
 }
 
@@ -98,25 +105,27 @@ __device__ __forceinline__ void hll_flux(const double L[5], const double R[5], d
     {
         const double gp = gamma * L[4];
         cL = gp * rsqrt(gp * L[0]);
-        const double k = fma(L[1], L[1], fma(L[2], L[2], L[3] * L[3]));
-        const double E = fma(0.5 * L[0], k, L[4] * igm1);
-        UL[0] = L[0]; UL[1] = L[0] * L[1]; UL[2] = L[0] * L[2]; UL[3] = L[0] * L[3]; UL[4] = E;
+        UL[0] = L[0]; UL[1] = L[0] * L[1]; UL[2] = L[0] * L[2]; UL[3] = L[0] * L[3];
+        const double rk = fma(UL[1], L[1], fma(UL[2], L[2], UL[3] * L[3]));     // rho |v|^2
+        const double E = fma(0.5, rk, L[4] * igm1);
+        UL[4] = E;
         FL[0] = UL[1]; FL[1] = fma(UL[1], L[1], L[4]); FL[2] = UL[2] * L[1]; FL[3] = UL[3] * L[1];
         FL[4] = (E + L[4]) * L[1];
     }
     {
         const double gp = gamma * R[4];
         cR = gp * rsqrt(gp * R[0]);
-        const double k = fma(R[1], R[1], fma(R[2], R[2], R[3] * R[3]));
-        const double E = fma(0.5 * R[0], k, R[4] * igm1);
-        UR[0] = R[0]; UR[1] = R[0] * R[1]; UR[2] = R[0] * R[2]; UR[3] = R[0] * R[3]; UR[4] = E;
+        UR[0] = R[0]; UR[1] = R[0] * R[1]; UR[2] = R[0] * R[2]; UR[3] = R[0] * R[3];
+        const double rk = fma(UR[1], R[1], fma(UR[2], R[2], UR[3] * R[3]));
+        const double E = fma(0.5, rk, R[4] * igm1);
+        UR[4] = E;
         FR[0] = UR[1]; FR[1] = fma(UR[1], R[1], R[4]); FR[2] = UR[2] * R[1]; FR[3] = UR[3] * R[1];
         FR[4] = (E + R[4]) * R[1];
     }
-    const double ap = dmax(0.0, dmax(L[1] + cL, R[1] + cR));
-    const double am = dmax(0.0, dmax(cL - L[1], cR - R[1]));
+    const double ap = max0(dmax(L[1] + cL, R[1] + cR));
+    const double am = max0(dmax(cL - L[1], cR - R[1]));
     const double w = rcp(ap + am);
-    const double al = ap * w, be = am * w, de = (ap * am) * w;
+    const double al = ap * w, be = am * w, de = al * am;
 #pragma unroll
     for (int v = 0; v < 5; ++v) {
         const double f = fma(al, FL[v], be * FR[v]);

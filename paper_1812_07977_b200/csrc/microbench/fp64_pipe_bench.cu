@@ -143,7 +143,7 @@ int main()
     double *res; cudaMalloc(&res, 4 * sizeof(double)); cudaMemset(res, 0, 32);
     acc<<<296, 256>>>(res, 1 << 26);
     double h[4]; cudaMemcpy(h, res, 32, cudaMemcpyDeviceToHost);
-    printf("max err: rcp(2 NR) %.3f ulp, rcp(1 NR) %.3g ulp, rsqrt(3rd+NR) %.3f (x q^2-1)/eps, rsqrt(3rd only) %.3f\n", h[0], h[1], h[2], h[3]);
+    printf("max err: rcp(production: seed + one third-order step) %.3f ulp, rcp(1 NR) %.3g ulp, rsqrt(3rd+NR) %.3f (x q^2-1)/eps, rsqrt(3rd only) %.3f\n", h[0], h[1], h[2], h[3]);
     {
         long long *cyc, h[64]; cudaMalloc(&cyc, 64 * 8);
         const int iters = 2000;
