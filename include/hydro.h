@@ -68,12 +68,26 @@ enum {
 int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6],
                  hydro_t **out);
 
+/* The paper's RiemannProblem also runs in one and two dimensions (Fig. 1, PAPER.md:138:
+ * "an extension of the classic 1D Sod shock tube ... to 2D and 3D"): hydro_create_nd makes a run of
+ * dimension ndim = 1, 2 or 3 whose first ndim axes are active, with cell edges d[0..ndim-1]
+ * (R21-R24).  An inactive axis has n[a] == 1, no ghost layers, no ghost exchange and no
+ * differences, reconstruction or fluxes (its d[a] and bc entries are ignored); all five variables
+ * are still carried.  The update is -(dt/dx) [dFx + (dx/dy) dFy + (dx/dz) dFz] over the active axes
+ * and hydro_cfl_dt returns (cfl/ndim) * min_d(d[a]) / max(|v| + c_s).  hydro_create(nx,ny,nz,..,dx,..)
+ * is hydro_create_nd(3, {nx,ny,nz}, {dx,dx,dx}, ..).  The packed layout stays U[5][nz][ny][nx].
+ * HYDRO_ERR_ARG if ndim is not 1..3, an active axis has n[a] < 2 or d[a] <= 0, an inactive axis has
+ * n[a] != 1, or the bc of an active axis is invalid. */
+int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, const int bc[6],
+                    hydro_t **out);
+
 /* Copy a packed state (host or device pointer, layout above) into the device state; resets the
  * time to 0 and the step count to 0.  Synchronises the handle's stream. */
 int hydro_set_state(hydro_t *h, const double *U);
 
 /* Algorithm 1 line 5, "ComputeTimeStep": reduction over active cells,
- *   *dt = (cfl/3) * (dx / max(|v| + c_s))      (R8; |v| Euclidean, c_s = sqrt(gamma p/rho)).
+ *   *dt = (cfl/3) * (dx / max(|v| + c_s))      (R8; |v| Euclidean, c_s = sqrt(gamma p/rho);
+ *                                               in general (cfl/ndim) * min_d(d[a]) / max, R22).
  * dt: host pointer.  Synchronises.  HYDRO_ERR_UNPHYSICAL if any active cell has rho <= 0,
  * p <= 0 or a non-finite speed. */
 int hydro_cfl_dt(hydro_t *h, double *dt);
@@ -120,7 +134,8 @@ int hydro_set_allocator(void *(*alloc)(size_t bytes, void *stream), void (*relea
  * host-side ComputeTimeStep of Algorithm 2). */
 int hydro_run_steps(hydro_t *h, long long n);
 /* Test hooks: run only the ghost fill on the current state, and read the padded buffer
- * [5][nz+4][ny+4][nx+4] (x fastest, row pitch removed) into a host or device array. */
+ * [5][nz+4][ny+4][nx+4] (x fastest, row pitch removed; no +4 on an inactive axis) into a host or
+ * device array. */
 int hydro_ghost_fill(hydro_t *h);
 int hydro_get_padded(hydro_t *h, double *Upad);
 /* Tuning hooks of the fused stage kernel (tests and measurement; defaults are chosen per grid).
@@ -132,14 +147,17 @@ int hydro_get_padded(hydro_t *h, double *Upad);
 int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk);
 int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long long *blocks);
 int hydro_set_graph_replay(hydro_t *h, int enable);
-/* Select the stage-kernel implementation: 0 = reference-structured simple kernel
- * (one thread per cell, everything recomputed), 1 = fused tiled kernel (default). */
+/* Select the stage-kernel implementation: 0 = reference-structured simple kernel (one thread per
+ * cell, everything recomputed, ghost layers filled in memory before each substep); 1 = fused tiled
+ * kernel with the boundary rules applied in the kernel (default: ghost layers are written to memory
+ * only for periodic x / y faces, and not at all otherwise -- three launches per step); 2 = the same
+ * fused kernel reading every ghost layer from memory (cross-check of 1). */
 int hydro_set_kernel_variant(hydro_t *h, int variant);
 /* Measurement hooks (bench.py): when enabled, every kernel launch of this handle is bracketed by
  * CUDA events on the handle's stream.  hydro_get_kernel_time synchronises and returns the summed
  * duration (ms) and launch count since profiling was enabled, for which = 0 ghost fill,
- * 1 stage-1 kernel, 2 stage-2 kernel, 3 (unused: the time-step update is folded into the first ghost fill
- * of a device-dt step), 4 stand-alone CFL reduction. */
+ * 1 stage-1 kernel, 2 stage-2 kernel, 3 start-of-step kernel (time step and accumulator reset, when
+ * the step has no ghost fill to carry them), 4 stand-alone CFL reduction. */
 int hydro_set_profiling(hydro_t *h, int enable);
 int hydro_get_kernel_time(hydro_t *h, int which, double *ms, long long *count);
 /* Number of kernels this library has launched since load (for bench.py's gpu_launches). */

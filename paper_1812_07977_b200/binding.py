@@ -16,7 +16,7 @@ _ERR = {1: "HYDRO_ERR_ARG", 2: "HYDRO_ERR_ALLOC", 3: "HYDRO_ERR_CUDA", 4: "HYDRO
         5: "HYDRO_ERR_NOSTATE"}
 
 # every symbol include/hydro.h declares (tests check the library exports all of them)
-SYMBOLS = ["hydro_create", "hydro_set_state", "hydro_cfl_dt", "hydro_step", "hydro_evolve",
+SYMBOLS = ["hydro_create", "hydro_create_nd", "hydro_set_state", "hydro_cfl_dt", "hydro_step", "hydro_evolve",
            "hydro_get_state", "hydro_destroy", "hydro_set_cfl", "hydro_set_limiter_theta",
            "hydro_get_time", "hydro_max_signal_speed", "hydro_set_stream", "hydro_set_allocator",
            "hydro_run_steps", "hydro_ghost_fill", "hydro_get_padded", "hydro_set_kernel_variant",
@@ -55,6 +55,8 @@ def load_library(verify=False):
     vp = C.c_void_p
     L.hydro_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double,
                                C.POINTER(C.c_int), C.POINTER(vp)]
+    L.hydro_create_nd.argtypes = [C.c_int, C.POINTER(C.c_int), _dp, C.c_double,
+                                  C.POINTER(C.c_int), C.POINTER(vp)]
     L.hydro_set_state.argtypes = [vp, vp]
     L.hydro_get_state.argtypes = [vp, vp]
     L.hydro_get_padded.argtypes = [vp, vp]
@@ -140,7 +142,7 @@ class Hydro:
     """hydro_t with the C-ABI's call names.  `verify=True` loads the -fmad=false build."""
 
     def __init__(self, nx, ny, nz, gamma, dx, bc, verify=False, torch_allocator=True,
-                 stream=None):
+                 stream=None, ndim=None, dxyz=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: this library has no CPU fallback")
@@ -148,10 +150,17 @@ class Hydro:
         torch.cuda.init()
         use_torch_allocator(self._L, bool(torch_allocator))
         self.shape = (5, nz, ny, nx)
-        self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
         self._h = C.c_void_p()
         arr = (C.c_int * 6)(*[int(b) for b in bc])
-        self._chk(self._L.hydro_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "hydro_create")
+        if ndim is None:                                   # 3D run, cubic cells
+            self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
+            self._chk(self._L.hydro_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "hydro_create")
+        else:                                              # run of dimension ndim, cell edges dxyz
+            g = [4 if a < ndim else 0 for a in range(3)]
+            self.padded_shape = (5, nz + g[2], ny + g[1], nx + g[0])
+            n = (C.c_int * 3)(nx, ny, nz)
+            d = (C.c_double * 3)(*(dxyz if dxyz is not None else (dx, dx, dx)))
+            self._chk(self._L.hydro_create_nd(ndim, n, d, gamma, arr, C.byref(self._h)), "hydro_create_nd")
         # The library enqueues on one stream.  By default that is a torch stream of the handle's own:
         # torch's default stream is the legacy stream 0, which cannot be captured, and
         # hydro_run_steps / hydro_evolve replay a captured CUDA graph.  Device tensors handed to

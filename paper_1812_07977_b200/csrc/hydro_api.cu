@@ -48,7 +48,9 @@ int fail(int code, const char *fmt, const char *a = "", const char *b = "")
 
 struct hydro {
     Grid g;
-    double dx, cfl;
+    double dx, cfl;                 // dx = edge along x (dt/dx scales the update)
+    double dxyz[3] = { 0, 0, 0 };   // cell edges; dmin = the smallest one over the active axes (R22)
+    double dmin = 0.0;
     double *block = nullptr;        // one allocation: [A | B]
     double *A = nullptr, *B = nullptr;   // element (0,0,0) of variable 0 of each buffer
     size_t buf_doubles = 0;         // doubles per buffer incl. lead
@@ -141,15 +143,40 @@ int is_device_pointer(const void *p, bool *on_device)
     return HYDRO_OK;
 }
 
-int launch_ghost_fill(hydro *h, double *U, bool clear_smax, bool advance_dt = false)
+// Which axes still get their ghost layers written to memory before a stage (GhostExchange,
+// PAPER.md:152, 172, 186).  The fused stage kernel applies outflow and reflecting rules itself and
+// serves every z ghost plane by remapping the TMA plane coordinate, so only periodic x / y faces
+// need the fill kernel; variant 2 (fused kernel reading memory ghosts) and the simple kernel need all.
+int fill_axes(const hydro *h)
+{
+    if (h->g.ndim < 3) return (1 << h->g.ndim) - 1;      // 1D / 2D runs: simple kernel, active axes only
+    if (h->variant != 1) return 7;
+    int axes = 0;
+    if (h->g.bc[0] == HYDRO_BC_PERIODIC) axes |= 1;
+    if (h->g.bc[2] == HYDRO_BC_PERIODIC) axes |= 2;
+    return axes;
+}
+
+int launch_ghost_fill(hydro *h, double *U, bool clear_smax, bool advance_dt = false, int axes = 7)
 {
     const Grid &g = h->g;
-    const long long n = (long long)g.nx * g.ny + (long long)g.ny * g.nz + (long long)g.nz * g.nx;
+    axes &= (1 << g.ndim) - 1;                               // inactive axes have no ghost layers
+    const long long n = ((axes & 4) ? (long long)g.nx * g.ny : 0) + ((axes & 1) ? (long long)g.ny * g.nz : 0) +
+                        ((axes & 2) ? (long long)g.nz * g.nx : 0);
     const int tb = 128;
     Scope sc(h, K_GHOST);
     ghost_fill_kernel<<<dim3((unsigned)((n + tb - 1) / tb), NVAR), tb, 0, h->stream>>>(
-        g, U, clear_smax ? &h->scal->smax_bits : nullptr, advance_dt ? h->scal : nullptr, h->cfl, h->dx);
+        g, U, clear_smax ? &h->scal->smax_bits : nullptr, advance_dt ? h->scal : nullptr,
+        h->cfl / (double)g.ndim, h->dmin, axes);
     LAUNCH_CHECK("ghost_fill");
+    return HYDRO_OK;
+}
+
+int launch_begin_step(hydro *h, bool advance_dt)
+{
+    Scope sc(h, K_NEXTDT);
+    begin_step_kernel<<<1, 1, 0, h->stream>>>(h->scal, advance_dt ? 1 : 0, h->cfl / (double)h->g.ndim, h->dmin);
+    LAUNCH_CHECK("begin_step");
     return HYDRO_OK;
 }
 
@@ -158,6 +185,7 @@ int launch_cfl_reduce(hydro *h)
     CUDA_TRY(cudaMemsetAsync(&h->scal->smax_bits, 0, sizeof(unsigned long long), h->stream));
     const long long rows = (long long)h->g.ny * h->g.nz;
     long long blocks = (rows + 7) / 8;
+    if (rows == 1) blocks = (h->g.nx + 255) / 256;          // 1D run: the warps of all blocks stride one row
     if (blocks > 148 * 8) blocks = 148 * 8;
     Scope sc(h, K_CFL);
     cfl_reduce_kernel<<<(unsigned)blocks, 256, 0, h->stream>>>(h->g, h->A, &h->scal->smax_bits,
@@ -175,14 +203,18 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
     const StepScalars *dd = dev_dt ? h->scal : nullptr;
     StepScalars *red = reduce ? h->scal : nullptr;
     Scope sc(h, STAGE == 1 ? K_STAGE1 : K_STAGE2);
-    if (h->variant == 0) {
+    if (h->variant == 0 || g.ndim < 3) {      // (variants 1 and 2 are the fused kernel, 3D runs only)
         dim3 tb(32, 4, 1);
-        dim3 gr((g.nx + 31) / 32, (g.ny + 3) / 4, g.nz);
-        stage_simple_kernel<STAGE><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
+        if (g.ndim == 1) tb = dim3(128, 1, 1);
+        dim3 gr((g.nx + tb.x - 1) / tb.x, (g.ny + tb.y - 1) / tb.y, g.nz);
+        if (g.ndim == 1)      stage_simple_kernel<STAGE, 1><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
+        else if (g.ndim == 2) stage_simple_kernel<STAGE, 2><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
+        else                  stage_simple_kernel<STAGE, 3><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
         LAUNCH_CHECK("stage_simple");
         return HYDRO_OK;
     }
-    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, h->stream);
+    const int inbc = h->variant == 1 ? 7 & ~fill_axes(h) : 0;
+    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused: %s%s", cudaGetErrorString(e));
     return HYDRO_OK;
@@ -193,10 +225,18 @@ int enqueue_step(hydro *h, double dt_host, bool dev_dt)
 {
     const double r = dt_host / h->dx;
     int rc;
-    // device dt: the first fill of the step also forms dt = (cfl/3) dx / smax and advances the clock
-    if ((rc = launch_ghost_fill(h, h->A, false, dev_dt))) return rc;
-    if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
-    if ((rc = launch_ghost_fill(h, h->B, true))) return rc;
+    const int axes = fill_axes(h);
+    if (axes) {
+        // device dt: the first fill of the step also forms dt = (cfl/3) dx / smax and advances the
+        // clock; the second one clears the accumulator of the reduction fused into stage 2
+        if ((rc = launch_ghost_fill(h, h->A, false, dev_dt, axes))) return rc;
+        if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
+        if ((rc = launch_ghost_fill(h, h->B, true, false, axes))) return rc;
+    } else {
+        // every boundary is applied inside the stage kernels: three launches per step
+        if ((rc = launch_begin_step(h, dev_dt))) return rc;
+        if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
+    }
     if ((rc = launch_stage<2>(h, h->B, h->A, h->A, r, dev_dt, true))) return rc;
     h->smax_valid = true;
     return HYDRO_OK;
@@ -234,11 +274,11 @@ int copy_state(hydro *h, double *padded, double *packed, bool to_padded)
         cudaMemcpy3DParms p;
         memset(&p, 0, sizeof p);
         cudaPitchedPtr dp = make_cudaPitchedPtr(padded + v * g.sv, (size_t)g.px * sizeof(double),
-                                                (size_t)g.px, (size_t)g.ny + 4);
+                                                (size_t)g.px, (size_t)g.ny + 2 * g.oy);
         cudaPitchedPtr hp = make_cudaPitchedPtr(packed + (size_t)v * g.nx * g.ny * g.nz,
                                                 (size_t)g.nx * sizeof(double), (size_t)g.nx,
                                                 (size_t)g.ny);
-        const cudaPos dpos = make_cudaPos(NG * sizeof(double), NG, NG);
+        const cudaPos dpos = make_cudaPos(NG * sizeof(double), g.oy, g.oz);
         const cudaPos hpos = make_cudaPos(0, 0, 0);
         if (to_padded) { p.srcPtr = hp; p.srcPos = hpos; p.dstPtr = dp; p.dstPos = dpos; }
         else           { p.srcPtr = dp; p.srcPos = dpos; p.dstPtr = hp; p.dstPos = hpos; }
@@ -347,19 +387,27 @@ int hydro_set_allocator(void *(*alloc)(size_t, void *), void (*release)(void *))
     return HYDRO_OK;
 }
 
-int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6], hydro_t **out)
+int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, const int bc[6],
+                    hydro_t **out)
 {
     if (!out) return fail(HYDRO_ERR_ARG, "create: out is NULL%s%s");
     *out = nullptr;
-    if (!bc) return fail(HYDRO_ERR_ARG, "create: bc is NULL%s%s");
-    if (nx < 2 || ny < 2 || nz < 2) return fail(HYDRO_ERR_ARG, "create: nx,ny,nz must be >= 2%s%s");
+    if (!bc || !n || !d) return fail(HYDRO_ERR_ARG, "create: NULL argument%s%s");
+    if (ndim < 1 || ndim > 3) return fail(HYDRO_ERR_ARG, "create: ndim must be 1, 2 or 3%s%s");
     if (!(gamma > 1.0) || !std::isfinite(gamma)) return fail(HYDRO_ERR_ARG, "create: gamma must be > 1%s%s");
-    if (!(dx > 0.0) || !std::isfinite(dx)) return fail(HYDRO_ERR_ARG, "create: dx must be > 0%s%s");
-    for (int f = 0; f < 6; ++f)
-        if (bc[f] < 0 || bc[f] > 2) return fail(HYDRO_ERR_ARG, "create: unknown boundary kind%s%s");
-    for (int a = 0; a < 3; ++a)
-        if ((bc[2 * a] == HYDRO_BC_PERIODIC) != (bc[2 * a + 1] == HYDRO_BC_PERIODIC))
-            return fail(HYDRO_ERR_ARG, "create: periodic must be set on both faces of an axis%s%s");
+    for (int a = 0; a < 3; ++a) {
+        if (a < ndim) {
+            if (n[a] < 2) return fail(HYDRO_ERR_ARG, "create: an active axis needs >= 2 cells%s%s");
+            if (!(d[a] > 0.0) || !std::isfinite(d[a])) return fail(HYDRO_ERR_ARG, "create: cell edges must be > 0%s%s");
+            if (bc[2 * a] < 0 || bc[2 * a] > 2 || bc[2 * a + 1] < 0 || bc[2 * a + 1] > 2)
+                return fail(HYDRO_ERR_ARG, "create: unknown boundary kind%s%s");
+            if ((bc[2 * a] == HYDRO_BC_PERIODIC) != (bc[2 * a + 1] == HYDRO_BC_PERIODIC))
+                return fail(HYDRO_ERR_ARG, "create: periodic must be set on both faces of an axis%s%s");
+        } else if (n[a] != 1) {
+            return fail(HYDRO_ERR_ARG, "create: an inactive axis must have exactly one cell%s%s");
+        }
+    }
+    const int nx = n[0], ny = n[1], nz = n[2];
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
@@ -370,13 +418,21 @@ int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6
     if (!h) return fail(HYDRO_ERR_ALLOC, "create: host allocation failed%s%s");
     Grid &g = h->g;
     g.nx = nx; g.ny = ny; g.nz = nz;
+    g.ndim = ndim; g.oy = ndim >= 2 ? NG : 0; g.oz = ndim >= 3 ? NG : 0;
     g.px = ((nx + 2 * NG + 15) / 16) * 16;
-    g.sy = (long long)g.px * (ny + 2 * NG);
-    const long long vol = g.sy * (nz + 2 * NG);
+    g.sy = (long long)g.px * (ny + 2 * g.oy);
+    const long long vol = g.sy * (nz + 2 * g.oz);
     g.sv = ((vol + 15) / 16) * 16;
-    memcpy(g.bc, bc, sizeof g.bc);
-    g.gamma = gamma; g.gm1 = gamma - 1.0; g.igm1 = 1.0 / g.gm1; g.theta = 1.4; g.r_dx = 0.0;
-    h->dx = dx; h->cfl = 0.7;
+    for (int f = 0; f < 6; ++f) g.bc[f] = f < 2 * ndim ? bc[f] : HYDRO_BC_OUTFLOW;
+    g.gamma = gamma; g.gm1 = gamma - 1.0; g.igm1 = 1.0 / g.gm1; g.theta = 1.4;
+    h->dx = d[0]; h->cfl = 0.7;
+    h->dmin = d[0];
+    for (int a = 0; a < 3; ++a) {
+        h->dxyz[a] = a < ndim ? d[a] : d[0];
+        if (a < ndim && d[a] < h->dmin) h->dmin = d[a];
+    }
+    g.ry = h->dx / h->dxyz[1]; g.rz = h->dx / h->dxyz[2];
+    if (ndim < 3) h->variant = 0;
     // +16 tail so vectorised / TMA reads that run a few doubles past the last row stay inside
     h->buf_doubles = (size_t)LEAD + (size_t)NVAR * g.sv + 16 + 2;
     h->buf_doubles = ((h->buf_doubles + 15) / 16) * 16;
@@ -390,7 +446,7 @@ int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6
     if (e == cudaSuccess) e = cudaMallocHost((void **)&h->scal_host, sizeof(StepScalars));
     if (e == cudaSuccess) e = cudaMemset(h->block, 0, 2 * h->buf_doubles * sizeof(double));
     if (e == cudaSuccess) e = cudaMemset(h->scal, 0, sizeof(StepScalars));
-    if (e == cudaSuccess) e = plan_stage_fused(h->plan, g, h->A, h->B);
+    if (e == cudaSuccess && ndim == 3) e = plan_stage_fused(h->plan, g, h->A, h->B);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();   // the memsets ran on the legacy stream; the handle's
                                                          // stream may be a non-blocking one
     if (e != cudaSuccess) {
@@ -401,6 +457,16 @@ int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6
     }
     *out = h;
     return HYDRO_OK;
+}
+
+int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6], hydro_t **out)
+{
+    if (out) *out = nullptr;
+    if (nx < 2 || ny < 2 || nz < 2) return fail(HYDRO_ERR_ARG, "create: nx,ny,nz must be >= 2%s%s");
+    if (!(dx > 0.0) || !std::isfinite(dx)) return fail(HYDRO_ERR_ARG, "create: dx must be > 0%s%s");
+    const int n[3] = { nx, ny, nz };
+    const double d[3] = { dx, dx, dx };
+    return hydro_create_nd(3, n, d, gamma, bc, out);
 }
 
 int hydro_destroy(hydro_t *h)
@@ -445,7 +511,9 @@ int hydro_set_limiter_theta(hydro_t *h, double theta)
 
 int hydro_set_kernel_variant(hydro_t *h, int variant)
 {
-    if (!h || variant < 0 || variant > 1) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0 or 1%s%s");
+    if (!h || variant < 0 || variant > 2) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0, 1 or 2%s%s");
+    if (h->g.ndim < 3 && variant != 0)
+        return fail(HYDRO_ERR_ARG, "set_kernel_variant: 1D / 2D runs use the simple kernel (variant 0)%s%s");
     h->variant = variant;
     drop_graph(h);
     return HYDRO_OK;
@@ -464,6 +532,7 @@ int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk)
     if (!h) return fail(HYDRO_ERR_ARG, "set_tiling: NULL handle%s%s");
     if ((tile_rows != 0 && tile_rows != 8 && tile_rows != 16) || planes_per_chunk < 0)
         return fail(HYDRO_ERR_ARG, "set_tiling: tile_rows must be 0, 8 or 16 and planes_per_chunk >= 0%s%s");
+    if (h->g.ndim < 3) return fail(HYDRO_ERR_ARG, "set_tiling: the fused kernel runs 3D grids only%s%s");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     drop_graph(h);
     h->ty_req = tile_rows; h->lz_req = planes_per_chunk;
@@ -515,7 +584,7 @@ int hydro_get_padded(hydro_t *h, double *Upad)
 {
     if (!h || !Upad) return fail(HYDRO_ERR_ARG, "get_padded: NULL argument%s%s");
     const Grid &g = h->g;
-    const size_t Nx = g.nx + 4, Ny = g.ny + 4, Nz = g.nz + 4;
+    const size_t Nx = g.nx + 2 * NG, Ny = g.ny + 2 * g.oy, Nz = g.nz + 2 * g.oz;
     for (int v = 0; v < NVAR; ++v)
         for (size_t K = 0; K < Nz; ++K)
             CUDA_TRY(cudaMemcpy2DAsync(Upad + ((size_t)v * Nz + K) * Ny * Nx, Nx * sizeof(double),
@@ -545,8 +614,8 @@ int hydro_cfl_dt(hydro_t *h, double *dt)
     double smax;
     int rc = hydro_max_signal_speed(h, &smax);
     if (rc) return rc;
-    const double c3 = h->cfl / 3.0;
-    const double dxs = h->dx / smax;
+    const double c3 = h->cfl / (double)h->g.ndim;
+    const double dxs = h->dmin / smax;
     *dt = c3 * dxs;
     return HYDRO_OK;
 }

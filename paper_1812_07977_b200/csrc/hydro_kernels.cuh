@@ -10,13 +10,15 @@ namespace hyd {
 // active cells I in [2, nx+1] etc.  `lead` doubles precede element (0,0,0) of every variable so
 // that the first active cell of every row sits on a 128-byte boundary.
 struct Grid {
-    int nx, ny, nz;          // active cells
+    int nx, ny, nz;          // active cells (1 on an inactive axis of a 1D / 2D run)
     int px;                  // row pitch (doubles)
-    long long sy;            // plane stride = px * (ny+4)
+    long long sy;            // plane stride = px * (ny + 2 oy)
     long long sv;            // variable stride (doubles), multiple of 16
     int bc[6];
     double gamma, gm1, igm1, theta;
-    double r_dx;             // unused by kernels that take dt/dx directly
+    int ndim;                // active axes: x | x,y | x,y,z  (R21)
+    int oy, oz;              // ghost layers per side in y and z: NG on an active axis, 0 otherwise (x: always NG)
+    double ry, rz;           // dx/dy, dx/dz: exactly 1 for cubic cells (R23)
 };
 
 __device__ __forceinline__ long long cell(const Grid &g, int I, int J, int K)
@@ -24,7 +26,13 @@ __device__ __forceinline__ long long cell(const Grid &g, int I, int J, int K)
     return (long long)I + (long long)g.px * J + g.sy * K;
 }
 
-// Device-resident time step (hydro_run_steps, hydro_evolve): dt = (cfl/3) * (dx / smax), clipped to
+// element (I, J, K) = first active cell of the padded arrays
+__device__ __forceinline__ long long cell0(const Grid &g, int i, int j, int k)
+{
+    return cell(g, i + NG, j + g.oy, k + g.oz);
+}
+
+// Device-resident time step (hydro_run_steps, hydro_evolve): dt = (cfl/ndim) * (dmin / smax), clipped to
 // land on t_final exactly (O8 / R14); once t_final is reached further steps get dt = 0, which the
 // stage kernels turn into the identity (U + (-(0*D)) = U, 0.5*((U+U)+(-0)) = U, bit for bit).
 struct StepScalars {
@@ -45,12 +53,13 @@ __global__ void begin_run_kernel(StepScalars *s, double t0, double t_final)
     s->done = 0;
 }
 
-__device__ __forceinline__ void advance_dt(StepScalars *s, double cfl, double dx)
+// `cfl_n` = CFL / ndim (formed on the host: one rounding), `dmin` = smallest edge of the cell (R22).
+__device__ __forceinline__ void advance_dt(StepScalars *s, double cfl_n, double dmin)
 {
     if (s->done) { s->dt = 0.0; return; }
     const double smax = __longlong_as_double((long long)s->smax_bits);
-    const double c3 = cfl / 3.0;
-    const double dxs = dx / smax;
+    const double c3 = cfl_n;
+    const double dxs = dmin / smax;
     double dt = __dmul_rn(c3, dxs);                    // never contracted: same roundings on every build
     const double t = s->t;
     if (__dadd_rn(t, dt) >= s->t_final) {
@@ -64,9 +73,14 @@ __device__ __forceinline__ void advance_dt(StepScalars *s, double cfl, double dx
     s->steps += 1;
 }
 
-// stand-alone form (kept for tests / other drivers); the step driver folds advance_dt into the
-// first ghost fill of the step, one launch less
-__global__ void next_dt_kernel(StepScalars *s, double cfl, double dx) { advance_dt(s, cfl, dx); }
+// Start of a step when no ghost fill is launched (every boundary is handled inside the stage
+// kernels): form this step's dt (device-dt steps) and clear the max-signal-speed accumulator for the
+// reduction fused into stage 2.  With a ghost fill in the step the same two jobs ride on it.
+__global__ void begin_step_kernel(StepScalars *s, int advance, double cfl_n, double dmin)
+{
+    if (advance) advance_dt(s, cfl_n, dmin);
+    s->smax_bits = 0ull;
+}
 
 // ------------------------------------------------------------------------------------------
 // A1 ghost fill (R9).  One thread per (face pair of one axis, transverse active cell); each
@@ -76,26 +90,28 @@ __global__ void next_dt_kernel(StepScalars *s, double cfl, double dx) { advance_
 // ------------------------------------------------------------------------------------------
 __global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
                                   unsigned long long *__restrict__ clear_smax,
-                                  StepScalars *advance, double cfl, double dx)
+                                  StepScalars *advance, double cfl_n, double dmin, int axes)
 {
     // first fill of a device-dt step: one thread also forms this step's dt (the stage kernels that
     // read it are launched after this kernel)
-    if (advance && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) advance_dt(advance, cfl, dx);
+    if (advance && blockIdx.x == 0 && blockIdx.y == 0 && threadIdx.x == 0) advance_dt(advance, cfl_n, dmin);
     // 32-bit index arithmetic (the three face counts are < 2^31 for any grid that fits the device)
-    const unsigned nxy = (unsigned)g.nx * g.ny, nyz = (unsigned)g.ny * g.nz, nzx = (unsigned)g.nz * g.nx;
+    // `axes`: bit a set = fill the ghost layers of axis a (the others are handled elsewhere)
+    const unsigned nxy = (axes & 4) ? (unsigned)g.nx * g.ny : 0u, nyz = (axes & 1) ? (unsigned)g.ny * g.nz : 0u,
+                   nzx = (axes & 2) ? (unsigned)g.nz * g.nx : 0u;
     unsigned t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t == 0 && blockIdx.y == 0 && clear_smax) *clear_smax = 0ull;
     int axis, n;
     long long base, stride;
     if (t < nxy) {                       // z faces: thread per (i,j), coalesced in i
         const int i = (int)(t % (unsigned)g.nx), j = (int)(t / (unsigned)g.nx);
-        axis = 2; n = g.nz; base = cell(g, i + NG, j + NG, 0); stride = g.sy;
+        axis = 2; n = g.nz; base = cell(g, i + NG, j + g.oy, 0); stride = g.sy;
     } else if ((t -= nxy) < nzx) {       // y faces: thread per (i,k), coalesced in i
         const int i = (int)(t % (unsigned)g.nx), k = (int)(t / (unsigned)g.nx);
-        axis = 1; n = g.ny; base = cell(g, i + NG, 0, k + NG); stride = g.px;
+        axis = 1; n = g.ny; base = cell(g, i + NG, 0, k + g.oz); stride = g.px;
     } else if ((t -= nzx) < nyz) {       // x faces: thread per (j,k)
         const int j = (int)(t % (unsigned)g.ny), k = (int)(t / (unsigned)g.ny);
-        axis = 0; n = g.nx; base = cell(g, 0, j + NG, k + NG); stride = 1;
+        axis = 0; n = g.nx; base = cell(g, 0, j + g.oy, k + g.oz); stride = 1;
     } else {
         return;
     }
@@ -205,7 +221,7 @@ cfl_reduce_kernel(Grid g, const double *__restrict__ U, unsigned long long *smax
     const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
     for (long long row = wglobal; row < nrow; row += nwarps) {
         const int j = (int)(row % g.ny), k = (int)(row / g.ny);
-        const double *u = U + cell(g, NG, j + NG, k + NG);
+        const double *u = U + cell0(g, 0, j, k);
         for (int i = lane; i < g.nx; i += 32) {
             const double c = cell_signal_speed(u[i], u[g.sv + i], u[2 * g.sv + i], u[3 * g.sv + i],
                                                u[4 * g.sv + i], g.gamma, g.gm1, bad);
@@ -265,7 +281,7 @@ __device__ __forceinline__ void flux_difference(const Grid &g, const double *__r
     dF[4] = Fp[4] - Fm[4];
 }
 
-template <int STAGE>
+template <int STAGE, int NDIM>
 __global__ void __launch_bounds__(128)
 stage_simple_kernel(Grid g, const double *__restrict__ Uin, const double *Uold, double *Uout,
                     double dt_over_dx, const StepScalars *__restrict__ dev_dt, double dx,
@@ -278,15 +294,25 @@ stage_simple_kernel(Grid g, const double *__restrict__ Uin, const double *Uold, 
     int bad = 0;
     if (i < g.nx && j < g.ny) {
         const double r = dev_dt ? dev_dt->dt / dx : dt_over_dx;
-        const long long c = cell(g, i + NG, j + NG, k + NG);
+        const long long c = cell0(g, i, j, k);
+        // flux differences of the active dimensions only (R21); those of y and z scaled by dx/dy and
+        // dx/dz (R23; exactly 1 for cubic cells)
         double dFx[5], dFy[5], dFz[5];
         flux_difference<0>(g, Uin, c, 1, dFx);
-        flux_difference<1>(g, Uin, c, g.px, dFy);
-        flux_difference<2>(g, Uin, c, g.sy, dFz);
+        if (NDIM >= 2) flux_difference<1>(g, Uin, c, g.px, dFy);
+        if (NDIM >= 3) flux_difference<2>(g, Uin, c, g.sy, dFz);
         double un[5];
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
-            const double D = sum3(dFx[v], dFy[v], dFz[v]);
+            double D = dFx[v];
+            if (NDIM == 2) {
+                const double ty = g.ry * dFy[v];
+                D = D + ty;
+            } else if (NDIM == 3) {
+                const double ty = g.ry * dFy[v];
+                const double tz = g.rz * dFz[v];
+                D = sum3(D, ty, tz);
+            }
             const double dU = -(r * D);
             if (STAGE == 1) {
                 un[v] = Uin[v * g.sv + c] + dU;
@@ -315,7 +341,7 @@ __global__ void repack_kernel(Grid g, double *padded, double *packed)
         const int i = (int)(t % g.nx);
         const long long jk = t / g.nx;
         const int j = (int)(jk % g.ny), k = (int)(jk / g.ny);
-        const long long c = cell(g, i + NG, j + NG, k + NG);
+        const long long c = cell0(g, i, j, k);
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) {
             if (TO_PADDED) padded[v * g.sv + c] = packed[v * nact + t];

@@ -12,9 +12,38 @@ struct FusedArgs {
     double dx;
     StepScalars *red;       // stage 2: max-signal-speed accumulator + sticky flag (or nullptr)
     int lz;                 // planes per z-chunk
+    int inbc;               // bit a: the boundary rule of axis a is applied by this kernel (ghost layers of
+                            // that axis are never read from memory); 0: all ghosts come from memory
 };
 
-// `umap` describes the stencil input (stage 1: U0, stage 2: U1; ghost-filled) to the TMA unit.
+// Boundary rule of one axis (O1 / R9) as an index map: the active cell whose state a ghost cell
+// takes (outflow: nearest active cell; reflecting: mirror image, normal momentum negated; periodic:
+// wrap).  i is an active-cell index; only the two ghost layers [-2,-1] and [n, n+1] matter, indices
+// further out are never used and are clamped into [cmin, cmax] (the caller's tile) to stay addressable.
+// Branch-free: the boundary kinds are uniform, the selects cost a handful of integer instructions.
+__device__ __forceinline__ int bc_source(int i, int n, int lo, int hi, int cmin, int cmax, bool &flip)
+{
+    const int below = lo == 0 ? 0 : (lo == 1 ? -1 - i : i + n);
+    const int above = hi == 0 ? n - 1 : (hi == 1 ? 2 * n - 1 - i : i - n);
+    flip = (i < 0 && lo == 1) || (i >= n && hi == 1);
+    const int s = i < 0 ? below : (i >= n ? above : i);
+    return min(max(s, cmin), cmax);
+}
+
+__device__ __forceinline__ double flip_sign(double x, bool f)
+{
+    return __hiloint2double(__double2hiint(x) ^ (f ? (int)0x80000000 : 0), __double2loint(x));
+}
+
+// `umap` describes the stencil input (stage 1: U0, stage 2: U1) to the TMA unit.
+//
+// Boundaries (GhostExchange of Algorithm 1).  Axes in `inbc` are handled here:
+// z ghost planes are never materialised -- the TMA plane coordinate is remapped to the source plane
+// (clamp / mirror / wrap); x and y ghost cells of outflow and reflecting faces are read from their
+// source cell inside the tile when the primitives are formed (own-cell source `wsrc` of the threads
+// that stand in for ghost cells, index map of the halo cells), with the normal momentum negated at
+// a wall.  Periodic x / y ghosts need cells from the far side of the domain and are still filled in
+// memory by ghost_fill_kernel (those axes are not in `inbc`).
 //
 // Synchronisation.  The x/y exchange of one plane needs block-wide hand-offs (primitives, outer
 // face values, fluxes).  Each is a split-phase mbarrier: a warp ARRIVES as soon as its stores are
@@ -28,7 +57,7 @@ struct FusedArgs {
 //   TY = 8 (two blocks per SM, single primitive tile):
 //     per cell plane c:  wait_W  x/y slopes  arrive_O  [prim(c+4), z-slope]  wait_O  fluxes  arrive_F
 //                        [z-flux, tile(c+1), arrive_W(c+1)]  wait_F  update
-template <int STAGE, int TY, int MINB>
+template <int STAGE, int TY, int MINB, bool ANISO>
 __global__ void __launch_bounds__(FTX * TY, MINB)
 stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 {
@@ -57,6 +86,29 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const bool active = (i0 + tx < g.nx) && (j0 + ty < g.ny);
     const long long col = (long long)(i0 + tx + NG) + (long long)g.px * (j0 + ty + NG);
     const int wc = (ty + 2) * WP + tx + 2;                    // own cell in a (tile + halo) plane
+    // Threads just past the active range stand in for the ghost cells of the domain's high faces:
+    // their primitives come from the ghost cell's source cell (in-kernel boundary rule).  Nothing of
+    // this is kept in registers: the map is recomputed by those (few, inactive) threads only, and
+    // the wall flags of z are block-uniform.
+    auto load_own = [&](const double *Ust, int p, double Un[5]) {
+        int ws = wc;
+        bool fx = false, fy = false;
+        if (!active && (a.inbc & 3)) {
+            const int is = (a.inbc & 1) ? bc_source(i0 + tx, g.nx, g.bc[0], g.bc[1], i0 - NG, i0 + TX + NG - 1, fx) : i0 + tx;
+            const int js = (a.inbc & 2) ? bc_source(j0 + ty, g.ny, g.bc[2], g.bc[3], j0 - NG, j0 + TY + NG - 1, fy) : j0 + ty;
+            ws = (js - j0 + NG) * WP + (is - i0 + NG);
+        }
+#pragma unroll
+        for (int v = 0; v < 5; ++v) Un[v] = Ust[v * S::WSZ + ws];
+        if (!active) { Un[1] = flip_sign(Un[1], fx); Un[2] = flip_sign(Un[2], fy); }
+        if ((a.inbc & 4) && (g.bc[4] == 1 || g.bc[5] == 1)) {  // a wall in z: mirror planes carry -m_z
+            const int kz = k0 + p - NG;                        // active z index of the plane
+            Un[3] = flip_sign(Un[3], (g.bc[4] == 1 && kz < 0) || (g.bc[5] == 1 && kz >= g.nz));
+        }
+    };
+    // tiles that touch a boundary handled here remap their halo cells (block-uniform)
+    const bool edge_tile = ((a.inbc & 1) && (i0 == 0 || i0 + TX + NG > g.nx)) ||
+                           ((a.inbc & 2) && (j0 == 0 || j0 + TY + NG > g.ny));
 
     // The tile's extra work (halo primitives, halo-cell slopes, high-edge faces) is a flattened
     // list handed out by ROLE = (warp + plane) mod TY, so that it rotates over the warps from plane
@@ -76,7 +128,10 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     __syncthreads();
     auto request_plane = [&](int p) {                         // thread 0 only
         tma::mbar_arrive_expect_tx(&bar[p % FNS], S::STAGE_BYTES);
-        tma::load_4d(sm + S::OFF_RING + (p % FNS) * S::STAGE, &umap, i0, j0, k0 + p, 0, &bar[p % FNS]);
+        // z ghost planes are never materialised: request the source plane instead (clamp / mirror / wrap)
+        bool fz;
+        const int K = (a.inbc & 4) ? bc_source(k0 + p - NG, g.nz, g.bc[4], g.bc[5], 0, g.nz - 1, fz) + NG : k0 + p;
+        tma::load_4d(sm + S::OFF_RING + (p % FNS) * S::STAGE, &umap, i0, j0, K, 0, &bar[p % FNS]);
     };
     if (t == 0)
         for (int p = 0; p < FNS; ++p) request_plane(p);       // nplanes >= 5 > FNS
@@ -93,9 +148,17 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             if (th < NHX) { const int q = th & 3; hr = (th >> 2) + 2; hc = q < 2 ? q : TX + q; }
             else { const int u = th - NHX, q = u / TX; hc = (u % TX) + 2; hr = q < 2 ? q : TY + q; }
             const int hw = hr * WP + hc;
+            int hs = hw;
+            bool fx = false, fy = false;
+            if (edge_tile) {
+                const int is = (a.inbc & 1) ? bc_source(i0 + hc - NG, g.nx, g.bc[0], g.bc[1], i0 - NG, i0 + TX + NG - 1, fx) : i0 + hc - NG;
+                const int js = (a.inbc & 2) ? bc_source(j0 + hr - NG, g.ny, g.bc[2], g.bc[3], j0 - NG, j0 + TY + NG - 1, fy) : j0 + hr - NG;
+                hs = (js - j0 + NG) * WP + (is - i0 + NG);
+            }
             double Uh[5], Wh[5];
 #pragma unroll
-            for (int v = 0; v < 5; ++v) Uh[v] = Uraw[v * S::WSZ + hw];
+            for (int v = 0; v < 5; ++v) Uh[v] = Uraw[v * S::WSZ + hs];
+            if (edge_tile) { Uh[1] = flip_sign(Uh[1], fx); Uh[2] = flip_sign(Uh[2], fy); }
             HYD_PRIM5(Uh, gm1, Wh);
 #pragma unroll
             for (int v = 0; v < 5; ++v) Wsm[v * S::WSZ + hw] = Wh[v];
@@ -118,8 +181,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     for (int p = 0; p < 4; ++p) {
         tma::mbar_wait(&bar[p], 0);
         double Un[5], Wn[5];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) Un[v] = sm[S::OFF_RING + p * S::STAGE + v * S::WSZ + wc];
+        load_own(sm + S::OFF_RING + p * S::STAGE, p, Un);
         HYD_PRIM5(Un, gm1, Wn);
         if (p >= 2) {
             double Iz[5], Ozn[5];
@@ -211,8 +273,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             const int p = c + 4;
             tma::mbar_wait(&bar[p % FNS], (p / FNS) & 1);
             double Un[5];
-#pragma unroll
-            for (int v = 0; v < 5; ++v) Un[v] = sm[S::OFF_RING + (p % FNS) * S::STAGE + v * S::WSZ + wc];
+            load_own(sm + S::OFF_RING + (p % FNS) * S::STAGE, p, Un);
             HYD_PRIM5(Un, gm1, Wn);
             HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
@@ -288,7 +349,8 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
         for (int v = 0; v < 5; ++v) {
             const double dFx = Fxs[v * S::XSZ + ty * XP + tx + 1] - Fxl[v];
-            const double dFy = Fys[v * S::YSZ + (ty + 1) * TX + tx] - Fyl[v];
+            double dFy = Fys[v * S::YSZ + (ty + 1) * TX + tx] - Fyl[v];
+            if (ANISO) { dFy = g.ry * dFy; dFz[v] = g.rz * dFz[v]; }    // non-cubic cells (R23): dx/dy, dx/dz
             const double D = HYD_SUM3(dFx, dFy, dFz[v]);
             const double dU = -(r * D);
             const double u1 = Uk[v * S::WSZ + wc];

@@ -16,9 +16,12 @@ struct FusedPlan {
 template <int STAGE, int TY, int MINB>
 inline cudaError_t fused_set_attr()
 {
-    return cudaFuncSetAttribute(stage_fused_kernel<STAGE, TY, MINB>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)FusedSmem<TY>::BYTES);
+    cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, TY, MINB, false>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)FusedSmem<TY>::BYTES);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(stage_fused_kernel<STAGE, TY, MINB, true>,
+                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FusedSmem<TY>::BYTES);
 }
 
 inline void fused_geometry(FusedPlan &p, const Grid &g, int ty, int lz)
@@ -79,18 +82,22 @@ template <int STAGE>
 inline cudaError_t launch_stage_fused(const FusedPlan &p, const Grid &g, const double *in,
                                       const double *old, double *out, double r,
                                       const StepScalars *dev_dt, double dx, StepScalars *red,
-                                      cudaStream_t stream)
+                                      int inbc, cudaStream_t stream)
 {
     if (!p.ready) return cudaErrorNotReady;
     const int b = in == p.base[0] ? 0 : 1;
     if (in != p.base[b]) return cudaErrorInvalidValue;
     FusedArgs a;
     a.g = g; a.Uold = old; a.Uout = out; a.dt_over_dx = r; a.dev_dt = dev_dt; a.dx = dx;
-    a.red = red; a.lz = p.lz;
-    if (p.ty == 16)
-        stage_fused_kernel<STAGE, 16, 1><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
-    else
-        stage_fused_kernel<STAGE, 8, 2><<<p.grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
+    a.red = red; a.lz = p.lz; a.inbc = inbc;
+    const bool aniso = g.ry != 1.0 || g.rz != 1.0;            // non-cubic cells: two more DMUL per variable
+    if (p.ty == 16) {
+        if (aniso) stage_fused_kernel<STAGE, 16, 1, true><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
+        else       stage_fused_kernel<STAGE, 16, 1, false><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
+    } else {
+        if (aniso) stage_fused_kernel<STAGE, 8, 2, true><<<p.grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
+        else       stage_fused_kernel<STAGE, 8, 2, false><<<p.grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
+    }
     return cudaGetLastError();
 }
 

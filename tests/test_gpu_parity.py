@@ -19,7 +19,7 @@ pytestmark = pytest.mark.gpu
 
 OUT, REF, PER = 0, 1, 2
 DEFAULT_VARIANT = int(os.environ.get("HYDRO_VARIANT", "1"))
-VARIANTS = [0, 1] if DEFAULT_VARIANT == 1 else [0]
+VARIANTS = [0, 1, 2] if DEFAULT_VARIANT == 1 else [0]
 
 
 def _mk(cls, shape, gamma, dx, bc, cfl=0.7, theta=None, **kw):
@@ -302,12 +302,13 @@ def test_fuzz_small_grids_bitwise():
         for _ in range(2):
             c.step(c.cfl_dt())
         want = c.get_state()
-        g = _gpu(shape, gamma, 1.0 / shape[0], bc, cfl, theta, verify=True)
-        g.set_tiling(ty, 0)
-        g.set_state(U); g.run_steps(2)
-        assert np.array_equal(g.get_state(), want), (case, shape, bc)
-        assert g.get_time() == c.get_time(), (case, shape, bc)
-        g.close()
+        for variant in (1, 2):          # boundary rules in the kernel / every ghost layer from memory
+            g = _gpu(shape, gamma, 1.0 / shape[0], bc, cfl, theta, verify=True, variant=variant)
+            g.set_tiling(ty, 0)
+            g.set_state(U); g.run_steps(2)
+            assert np.array_equal(g.get_state(), want), (case, variant, shape, bc)
+            assert g.get_time() == c.get_time(), (case, variant, shape, bc)
+            g.close()
         g = _gpu(shape, gamma, 1.0 / shape[0], bc, cfl, theta, verify=False)
         g.set_tiling(ty, 0)
         g.set_state(U); g.run_steps(2)
@@ -530,7 +531,7 @@ def test_status_codes():
         g.set_limiter_theta(0.5)
     n0 = g.launch_count()
     g.step(g.cfl_dt())
-    assert g.launch_count() >= n0 + 4
+    assert g.launch_count() >= n0 + 3            # all-outflow: start-of-step kernel + two stage kernels
 
 
 def test_uniform_state_bit_identical_on_production_build():
@@ -553,3 +554,24 @@ def test_deterministic_run_to_run():
         g.run_steps(8)
         outs.append(g.get_state())
     assert np.array_equal(outs[0], outs[1])
+
+
+def test_launches_per_step_follow_the_boundary_kinds():
+    """The fused kernel applies outflow / reflecting rules itself and remaps z ghost planes, so a step
+    is three launches (start-of-step, stage 1, stage 2) unless x or y is periodic (then the ghost fill
+    of those axes runs before each stage and carries the start-of-step work: four launches)."""
+    U = inputs.random_state(40, 12, 9, seed=2)
+    for bc, per_step in (((OUT,) * 6, 3), ((REF, OUT, OUT, REF, PER, PER), 3), ((PER, PER, OUT, OUT, OUT, OUT), 4),
+                         ((OUT, OUT, PER, PER, REF, REF), 4)):
+        g = _gpu((40, 12, 9), 1.4, 0.025, bc)
+        g.set_state(U)
+        g.run_steps(1)
+        n0 = g.launch_count()
+        g.run_steps(5)
+        assert g.launch_count() - n0 == 5 * per_step, (bc, g.launch_count() - n0)
+        g.set_kernel_variant(2)
+        g.run_steps(1)
+        n0 = g.launch_count()
+        g.run_steps(5)
+        assert g.launch_count() - n0 == 20
+        g.close()
