@@ -45,7 +45,11 @@ typedef struct hydro hydro_t;   /* opaque */
 
 /* Boundary rule per face (R9; replaces the physical-boundary part of the paper's
  * GhostExchange). */
-enum { HYDRO_BC_OUTFLOW = 0, HYDRO_BC_REFLECT = 1, HYDRO_BC_PERIODIC = 2 };
+enum { HYDRO_BC_OUTFLOW = 0, HYDRO_BC_REFLECT = 1, HYDRO_BC_PERIODIC = 2,
+       /* z faces only: the face is an interface to a neighbouring slab of a domain decomposed along
+        * z; its two ghost layers are written by the halo exchange (hydro_halo_*), never by the
+        * library's boundary code.  Set by hydro_create_slab. */
+       HYDRO_BC_NEIGHBOUR = 3 };
 
 enum {
     HYDRO_OK = 0,
@@ -133,6 +137,46 @@ int hydro_set_allocator(void *(*alloc)(size_t bytes, void *stream), void (*relea
  * theta or the kernel variant changes).  The benchmark path (Algorithm 1's loop body without the
  * host-side ComputeTimeStep of Algorithm 2). */
 int hydro_run_steps(hydro_t *h, long long n);
+/* ---- domain decomposition into z-slabs ----------------------------------------------------
+ * The paper runs the problem decomposed over MPI ranks, one GPU each, 256^3 cells per rank, with a
+ * ghost exchange after every Runge-Kutta substep and a reduction of the time step every step
+ * (PAPER.md:172, 186, 245, 264, 325, 357); its exchange goes through the host, and device-to-device
+ * exchange is named as future work.  Here a slab is an ordinary handle whose z faces
+ * towards neighbouring slabs have kind HYDRO_BC_NEIGHBOUR; a driver (paper_1812_07977_b200/slab.py)
+ * alternates hydro_substep with the exchange of the two boundary planes per interface and all-reduces
+ * the maximum signal speed.  Results are bit-identical to the single-domain run.
+ *
+ * hydro_create_slab: the handle of slab `rank` of `nranks` for a global nx*ny*nz_global grid with
+ * physical boundaries bc (cubic cells).  Planes are dealt out evenly, the first nz_global % nranks
+ * slabs getting one more; *k_first / *nz_local (may be NULL) receive the slab's first global plane
+ * and its plane count.  A periodic z boundary becomes a neighbour interface between the last and the
+ * first slab.  HYDRO_ERR_ARG if a slab would have fewer than 2 planes.
+ * hydro_substep: one substep (stage 1: U1 = U0 + dU(U0) into the second buffer; stage 2:
+ * U(n+1) = 0.5 (U0 + U1 + dU(U1)) in place, with the fused max-signal-speed reduction) on
+ * part 0 = all planes, 1 = the planes next to neighbour interfaces (launch these first, exchange
+ * them while part 2 runs), 2 = the remaining planes.  dt > 0: host-supplied step; dt == 0: the
+ * device-resident step (cfl/3) dx / smax formed at the start of stage 1 from the running maximum
+ * at hydro_smax_device, which the driver has all-reduced (MAX) over the slabs (hydro_reduce_smax
+ * computes the local value after hydro_set_state).  Asynchronous.
+ * hydro_halo_count: doubles in one packed face = 5 * 2 * ny * nx.  hydro_halo_pack copies the two
+ * ACTIVE planes next to face `side` (0 = z low, 1 = z high) of buffer `which` (0 = state, 1 = stage-1
+ * result) into dst[5][2][ny][nx] (device pointer); hydro_halo_unpack writes src into the two GHOST
+ * planes of that face.  hydro_halo_push does both at once as direct stores into the neighbour's
+ * state (device pointer from hydro_state_base on the neighbour, mapped on this device: same process,
+ * peer access or CUDA IPC) -- over NVLink when the neighbour lives on another GPU.  All asynchronous
+ * on the handle's stream; ordering between slabs (events, barriers) is the driver's. */
+int hydro_create_slab(int nx, int ny, int nz_global, double gamma, double dx, const int bc[6],
+                      int rank, int nranks, hydro_t **out, int *k_first, int *nz_local);
+int hydro_substep(hydro_t *h, int stage, double dt, int part);
+int hydro_halo_count(hydro_t *h, size_t *doubles);
+int hydro_halo_pack(hydro_t *h, int which, int side, double *dst);
+int hydro_halo_unpack(hydro_t *h, int which, int side, const double *src);
+int hydro_halo_push(hydro_t *h, int which, int side, double *peer_base, int peer_nz,
+                    long long peer_var_stride);
+int hydro_state_base(hydro_t *h, int which, double **base, int *nz_local, long long *var_stride);
+int hydro_smax_device(hydro_t *h, double **smax);
+int hydro_reduce_smax(hydro_t *h);
+
 /* Test hooks: run only the ghost fill on the current state, and read the padded buffer
  * [5][nz+4][ny+4][nx+4] (x fastest, row pitch removed; no +4 on an inactive axis) into a host or
  * device array. */

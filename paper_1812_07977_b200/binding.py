@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-BC_OUTFLOW, BC_REFLECT, BC_PERIODIC = 0, 1, 2
+BC_OUTFLOW, BC_REFLECT, BC_PERIODIC, BC_NEIGHBOUR = 0, 1, 2, 3
 _ERR = {1: "HYDRO_ERR_ARG", 2: "HYDRO_ERR_ALLOC", 3: "HYDRO_ERR_CUDA", 4: "HYDRO_ERR_UNPHYSICAL",
         5: "HYDRO_ERR_NOSTATE"}
 
@@ -21,6 +21,9 @@ SYMBOLS = ["hydro_create", "hydro_create_nd", "hydro_set_state", "hydro_cfl_dt",
            "hydro_get_time", "hydro_max_signal_speed", "hydro_set_stream", "hydro_set_allocator",
            "hydro_run_steps", "hydro_ghost_fill", "hydro_get_padded", "hydro_set_kernel_variant",
            "hydro_set_tiling", "hydro_get_tiling", "hydro_set_graph_replay",
+           "hydro_create_slab", "hydro_substep", "hydro_halo_count", "hydro_halo_pack",
+           "hydro_halo_unpack", "hydro_halo_push", "hydro_state_base", "hydro_smax_device",
+           "hydro_reduce_smax",
            "hydro_set_profiling", "hydro_get_kernel_time", "hydro_launch_count",
            "hydro_is_verification_build", "hydro_last_error"]
 
@@ -76,6 +79,16 @@ def load_library(verify=False):
     L.hydro_set_tiling.argtypes = [vp, C.c_int, C.c_int]
     L.hydro_get_tiling.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.hydro_set_graph_replay.argtypes = [vp, C.c_int]
+    L.hydro_create_slab.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int),
+                                    C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.hydro_substep.argtypes = [vp, C.c_int, C.c_double, C.c_int]
+    L.hydro_halo_count.argtypes = [vp, C.POINTER(C.c_size_t)]
+    L.hydro_halo_pack.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.hydro_halo_unpack.argtypes = [vp, C.c_int, C.c_int, vp]
+    L.hydro_halo_push.argtypes = [vp, C.c_int, C.c_int, vp, C.c_int, C.c_longlong]
+    L.hydro_state_base.argtypes = [vp, C.c_int, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
+    L.hydro_smax_device.argtypes = [vp, C.POINTER(vp)]
+    L.hydro_reduce_smax.argtypes = [vp]
     L.hydro_set_profiling.argtypes = [vp, C.c_int]
     L.hydro_get_kernel_time.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_longlong)]
     L.hydro_launch_count.restype = C.c_longlong
@@ -142,7 +155,9 @@ class Hydro:
     """hydro_t with the C-ABI's call names.  `verify=True` loads the -fmad=false build."""
 
     def __init__(self, nx, ny, nz, gamma, dx, bc, verify=False, torch_allocator=True,
-                 stream=None, ndim=None, dxyz=None):
+                 stream=None, ndim=None, dxyz=None, slab=None):
+        """`slab=(rank, nranks)`: the handle of one z-slab of the global nx*ny*nz grid
+        (hydro_create_slab); self.k_first / self.shape then describe the slab."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: this library has no CPU fallback")
@@ -152,7 +167,15 @@ class Hydro:
         self.shape = (5, nz, ny, nx)
         self._h = C.c_void_p()
         arr = (C.c_int * 6)(*[int(b) for b in bc])
-        if ndim is None:                                   # 3D run, cubic cells
+        self.k_first = 0
+        if slab is not None:
+            k0, nzl = C.c_int(), C.c_int()
+            self._chk(self._L.hydro_create_slab(nx, ny, nz, gamma, dx, arr, int(slab[0]), int(slab[1]),
+                                                C.byref(self._h), C.byref(k0), C.byref(nzl)), "hydro_create_slab")
+            self.k_first, nz = k0.value, nzl.value
+            self.shape = (5, nz, ny, nx)
+            self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
+        elif ndim is None:                                 # 3D run, cubic cells
             self.padded_shape = (5, nz + 4, ny + 4, nx + 4)
             self._chk(self._L.hydro_create(nx, ny, nz, gamma, dx, arr, C.byref(self._h)), "hydro_create")
         else:                                              # run of dimension ndim, cell edges dxyz
@@ -269,3 +292,35 @@ class Hydro:
 
     def launch_count(self):
         return self._L.hydro_launch_count()
+
+    # ---- z-slab decomposition (driver: paper_1812_07977_b200/slab.py) ----
+    def substep(self, stage, dt=0.0, part=0):
+        self._chk(self._L.hydro_substep(self._h, stage, dt, part), "hydro_substep")
+
+    def halo_count(self):
+        n = C.c_size_t()
+        self._chk(self._L.hydro_halo_count(self._h, C.byref(n)), "hydro_halo_count")
+        return n.value
+
+    def halo_pack(self, which, side, dst):
+        self._chk(self._L.hydro_halo_pack(self._h, which, side, C.c_void_p(dst.data_ptr())), "hydro_halo_pack")
+
+    def halo_unpack(self, which, side, src):
+        self._chk(self._L.hydro_halo_unpack(self._h, which, side, C.c_void_p(src.data_ptr())), "hydro_halo_unpack")
+
+    def state_base(self, which):
+        p, nz, sv = C.c_void_p(), C.c_int(), C.c_longlong()
+        self._chk(self._L.hydro_state_base(self._h, which, C.byref(p), C.byref(nz), C.byref(sv)), "hydro_state_base")
+        return p.value, nz.value, sv.value
+
+    def halo_push(self, which, side, peer_base, peer_nz, peer_var_stride):
+        self._chk(self._L.hydro_halo_push(self._h, which, side, C.c_void_p(peer_base), peer_nz, peer_var_stride),
+                  "hydro_halo_push")
+
+    def smax_device(self):
+        p = C.c_void_p()
+        self._chk(self._L.hydro_smax_device(self._h, C.byref(p)), "hydro_smax_device")
+        return p.value
+
+    def reduce_smax(self):
+        self._chk(self._L.hydro_reduce_smax(self._h), "hydro_reduce_smax")

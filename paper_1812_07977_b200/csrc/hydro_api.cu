@@ -195,26 +195,32 @@ int launch_cfl_reduce(hydro *h)
     return HYDRO_OK;
 }
 
+// One substep over the active planes [kb, ke) (whole grid: 0, nz).  The fused kernel works in
+// z-chunks of plan.lz planes, so kb and ke must be chunk boundaries (or nz).
 template <int STAGE>
 int launch_stage(hydro *h, const double *in, const double *old, double *out, double r,
-                 bool dev_dt, bool reduce)
+                 bool dev_dt, bool reduce, int kb = 0, int ke = -1)
 {
     const Grid &g = h->g;
+    if (ke < 0) ke = g.nz;
+    if (ke <= kb) return HYDRO_OK;
     const StepScalars *dd = dev_dt ? h->scal : nullptr;
     StepScalars *red = reduce ? h->scal : nullptr;
     Scope sc(h, STAGE == 1 ? K_STAGE1 : K_STAGE2);
     if (h->variant == 0 || g.ndim < 3) {      // (variants 1 and 2 are the fused kernel, 3D runs only)
         dim3 tb(32, 4, 1);
         if (g.ndim == 1) tb = dim3(128, 1, 1);
-        dim3 gr((g.nx + tb.x - 1) / tb.x, (g.ny + tb.y - 1) / tb.y, g.nz);
-        if (g.ndim == 1)      stage_simple_kernel<STAGE, 1><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
-        else if (g.ndim == 2) stage_simple_kernel<STAGE, 2><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
-        else                  stage_simple_kernel<STAGE, 3><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red);
+        dim3 gr((g.nx + tb.x - 1) / tb.x, (g.ny + tb.y - 1) / tb.y, ke - kb);
+        if (g.ndim == 1)      stage_simple_kernel<STAGE, 1><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red, kb);
+        else if (g.ndim == 2) stage_simple_kernel<STAGE, 2><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red, kb);
+        else                  stage_simple_kernel<STAGE, 3><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red, kb);
         LAUNCH_CHECK("stage_simple");
         return HYDRO_OK;
     }
     const int inbc = h->variant == 1 ? 7 & ~fill_axes(h) : 0;
-    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream);
+    const int lz = h->plan.lz;
+    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream,
+                                              kb / lz, (ke - kb + lz - 1) / lz);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused: %s%s", cudaGetErrorString(e));
     return HYDRO_OK;
@@ -399,7 +405,8 @@ int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, c
         if (a < ndim) {
             if (n[a] < 2) return fail(HYDRO_ERR_ARG, "create: an active axis needs >= 2 cells%s%s");
             if (!(d[a] > 0.0) || !std::isfinite(d[a])) return fail(HYDRO_ERR_ARG, "create: cell edges must be > 0%s%s");
-            if (bc[2 * a] < 0 || bc[2 * a] > 2 || bc[2 * a + 1] < 0 || bc[2 * a + 1] > 2)
+            const int kmax = a == 2 ? HYDRO_BC_NEIGHBOUR : HYDRO_BC_PERIODIC;   // slabs are cut along z
+            if (bc[2 * a] < 0 || bc[2 * a] > kmax || bc[2 * a + 1] < 0 || bc[2 * a + 1] > kmax)
                 return fail(HYDRO_ERR_ARG, "create: unknown boundary kind%s%s");
             if ((bc[2 * a] == HYDRO_BC_PERIODIC) != (bc[2 * a + 1] == HYDRO_BC_PERIODIC))
                 return fail(HYDRO_ERR_ARG, "create: periodic must be set on both faces of an axis%s%s");
@@ -687,6 +694,169 @@ int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
     h->step += h->scal_host->steps;
     h->t_on_device = false;
     if (nsteps) *nsteps = h->scal_host->steps;
+    return HYDRO_OK;
+}
+
+// ---- slab decomposition along z ------------------------
+
+int hydro_create_slab(int nx, int ny, int nz_global, double gamma, double dx, const int bc[6],
+                      int rank, int nranks, hydro_t **out, int *k_first, int *nz_local)
+{
+    if (out) *out = nullptr;
+    if (!out || !bc) return fail(HYDRO_ERR_ARG, "create_slab: NULL argument%s%s");
+    if (nranks < 1 || rank < 0 || rank >= nranks) return fail(HYDRO_ERR_ARG, "create_slab: bad rank%s%s");
+    if (nz_global < 2 * nranks) return fail(HYDRO_ERR_ARG, "create_slab: every slab needs >= 2 planes%s%s");
+    for (int f = 0; f < 6; ++f)
+        if (bc[f] < 0 || bc[f] > 2) return fail(HYDRO_ERR_ARG, "create_slab: unknown boundary kind%s%s");
+    // planes [k0, k0 + nzl): the first nz_global % nranks slabs get one plane more
+    const int base = nz_global / nranks, extra = nz_global % nranks;
+    const int nzl = base + (rank < extra ? 1 : 0);
+    const int k0 = rank * base + (rank < extra ? rank : extra);
+    int b[6];
+    memcpy(b, bc, sizeof b);
+    const bool periodic_z = bc[4] == HYDRO_BC_PERIODIC;
+    if (nranks > 1) {
+        if (rank > 0 || periodic_z) b[4] = HYDRO_BC_NEIGHBOUR;
+        if (rank < nranks - 1 || periodic_z) b[5] = HYDRO_BC_NEIGHBOUR;
+    }
+    if (k_first) *k_first = k0;
+    if (nz_local) *nz_local = nzl;
+    if (nx < 2 || ny < 2) return fail(HYDRO_ERR_ARG, "create_slab: nx,ny must be >= 2%s%s");
+    const int n[3] = { nx, ny, nzl };
+    const double d[3] = { dx, dx, dx };
+    return hydro_create_nd(3, n, d, gamma, b, out);
+}
+
+int hydro_halo_count(hydro_t *h, size_t *doubles)
+{
+    if (!h || !doubles) return fail(HYDRO_ERR_ARG, "halo_count: NULL argument%s%s");
+    *doubles = (size_t)NVAR * 2 * h->g.ny * h->g.nx;
+    return HYDRO_OK;
+}
+
+namespace {
+int halo_blocks(const hydro *h)
+{
+    const long long total = 10ll * h->g.ny * h->g.nx;
+    long long b = (total + 255) / 256;
+    return (int)(b > 148 * 8 ? 148 * 8 : b);
+}
+int halo_args(hydro *h, int which, int side, const void *p, const char *who)
+{
+    if (!h || !p || (which != 0 && which != 1) || (side != 0 && side != 1))
+        return fail(HYDRO_ERR_ARG, "%s: bad argument%s", who);
+    if (h->g.ndim != 3) return fail(HYDRO_ERR_ARG, "%s: slabs are cut along z of a 3D run%s", who);
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "%s before set_state%s", who);
+    return HYDRO_OK;
+}
+}  // namespace
+
+int hydro_halo_pack(hydro_t *h, int which, int side, double *dst)
+{
+    int rc = halo_args(h, which, side, dst, "halo_pack");
+    if (rc) return rc;
+    const Grid &g = h->g;
+    halo_kernel<0><<<halo_blocks(h), 256, 0, h->stream>>>(g, which ? h->B : h->A, dst, side ? g.nz : NG, 0, 0);
+    LAUNCH_CHECK("halo_pack");
+    return HYDRO_OK;
+}
+
+int hydro_halo_unpack(hydro_t *h, int which, int side, const double *src)
+{
+    int rc = halo_args(h, which, side, src, "halo_unpack");
+    if (rc) return rc;
+    const Grid &g = h->g;
+    halo_kernel<1><<<halo_blocks(h), 256, 0, h->stream>>>(g, which ? h->B : h->A, const_cast<double *>(src),
+                                                          side ? g.nz + NG : 0, 0, 0);
+    LAUNCH_CHECK("halo_unpack");
+    return HYDRO_OK;
+}
+
+int hydro_state_base(hydro_t *h, int which, double **base, int *nz_local, long long *var_stride)
+{
+    if (!h || !base || (which != 0 && which != 1)) return fail(HYDRO_ERR_ARG, "state_base: bad argument%s%s");
+    *base = which ? h->B : h->A;
+    if (nz_local) *nz_local = h->g.nz;
+    if (var_stride) *var_stride = h->g.sv;
+    return HYDRO_OK;
+}
+
+int hydro_halo_push(hydro_t *h, int which, int side, double *peer_base, int peer_nz, long long peer_var_stride)
+{
+    int rc = halo_args(h, which, side, peer_base, "halo_push");
+    if (rc) return rc;
+    const Grid &g = h->g;
+    // my low boundary planes fill the neighbour's HIGH ghost planes and vice versa
+    const int K0 = side ? g.nz : NG, Kd = side ? 0 : peer_nz + NG;
+    halo_kernel<2><<<halo_blocks(h), 256, 0, h->stream>>>(g, which ? h->B : h->A, peer_base, K0, Kd, peer_var_stride);
+    LAUNCH_CHECK("halo_push");
+    return HYDRO_OK;
+}
+
+int hydro_smax_device(hydro_t *h, double **smax)
+{
+    if (!h || !smax) return fail(HYDRO_ERR_ARG, "smax_device: NULL argument%s%s");
+    *smax = reinterpret_cast<double *>(&h->scal->smax_bits);
+    return HYDRO_OK;
+}
+
+int hydro_reduce_smax(hydro_t *h)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "reduce_smax: NULL handle%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "reduce_smax before set_state%s%s");
+    if (h->smax_valid) return HYDRO_OK;
+    return launch_cfl_reduce(h);
+}
+
+// One substep of the RK2 step on the planes of `part`, for drivers that put a halo exchange between
+// the substeps.  dt > 0: host-supplied step; dt == 0: the device-resident step, formed at the start
+// of substep 1 from the (all-reduced) running maximum.
+int hydro_substep(hydro_t *h, int stage, double dt, int part)
+{
+    if (!h || (stage != 1 && stage != 2) || part < 0 || part > 2 || !(dt >= 0.0) || !std::isfinite(dt))
+        return fail(HYDRO_ERR_ARG, "substep: bad argument%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "substep before set_state%s%s");
+    const Grid &g = h->g;
+    const bool dev_dt = dt == 0.0;
+    int rc;
+    if (dev_dt && !h->smax_valid) return fail(HYDRO_ERR_NOSTATE, "substep: device dt needs hydro_reduce_smax first%s%s");
+    if (dev_dt && !h->t_on_device && (rc = begin_run(h, HUGE_VAL))) return rc;
+    if (!dev_dt && h->t_on_device && (rc = read_scalars(h))) return rc;
+    const double r = dt / h->dx;
+    // interface planes: the z-chunks (fused kernel) or plane pairs (simple kernel) next to a
+    // neighbouring slab; computed first so that their exchange overlaps the interior
+    const int unit = (h->variant == 0 || g.ndim < 3) ? 2 : h->plan.lz;
+    int lo_end = 0, hi_begin = g.nz;
+    if (g.bc[4] == HYDRO_BC_NEIGHBOUR) lo_end = unit < g.nz ? unit : g.nz;
+    if (g.bc[5] == HYDRO_BC_NEIGHBOUR) {
+        hi_begin = ((g.nz - 1) / unit) * unit;                   // start of the last chunk ...
+        if (g.nz - hi_begin < 2 && hi_begin >= unit) hi_begin -= unit;   // ... which must hold two planes
+    }
+    if (hi_begin < lo_end) hi_begin = lo_end;
+    const bool first = part != 2;                                // the launch that opens the substep
+    if (stage == 1 && first) {
+        const int axes = fill_axes(h);
+        if (axes) { if ((rc = launch_ghost_fill(h, h->A, true, dev_dt, axes))) return rc; }
+        else if ((rc = launch_begin_step(h, dev_dt))) return rc;
+    }
+    if (stage == 2 && first) {
+        const int axes = fill_axes(h);
+        if (axes && (rc = launch_ghost_fill(h, h->B, false, false, axes))) return rc;
+    }
+    const double *in = stage == 1 ? h->A : h->B;
+    const double *old = stage == 1 ? nullptr : h->A;
+    double *outp = stage == 1 ? h->B : h->A;
+    auto run = [&](int kb, int ke) {
+        return stage == 1 ? launch_stage<1>(h, in, old, outp, r, dev_dt, false, kb, ke)
+                          : launch_stage<2>(h, in, old, outp, r, dev_dt, true, kb, ke);
+    };
+    if (part == 0) { if ((rc = run(0, g.nz))) return rc; }
+    else if (part == 1) { if ((rc = run(0, lo_end))) return rc; if ((rc = run(hi_begin, g.nz))) return rc; }
+    else { if ((rc = run(lo_end, hi_begin))) return rc; }
+    if (stage == 2 && (part == 0 || part == 2)) {                // the step is complete
+        h->smax_valid = true;
+        if (!dev_dt) { h->t = h->t + dt; h->step += 1; }
+    }
     return HYDRO_OK;
 }
 

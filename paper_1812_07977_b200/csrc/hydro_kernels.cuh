@@ -133,7 +133,7 @@ __global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
             double2 gl, gh;
             if (lo == 0)      { gl.x = l2.x; gl.y = l2.x; }
             else if (lo == 1) { gl.x = sgn * l2.y; gl.y = sgn * l2.x; }
-            else              { gl = h2; }
+            else              { gl = h2; }                   // (x is never a slab interface)
             if (hi == 0)      { gh.x = h2.y; gh.y = h2.y; }
             else if (hi == 1) { gh.x = sgn * h2.y; gh.y = sgn * h2.x; }
             else              { gh = l2; }
@@ -156,8 +156,9 @@ __global__ void ghost_fill_kernel(Grid g, double *__restrict__ U,
         if (hi == 0)      { g2 = an1; g3 = an1; }
         else if (hi == 1) { g2 = sgn * an1; g3 = sgn * an; }
         else              { g2 = a2; g3 = a3; }
-        a[0] = g0; a[stride] = g1;
-        a[(long long)(n + 2) * stride] = g2; a[(long long)(n + 3) * stride] = g3;
+        // kind 3 (neighbouring slab, z only): those ghost layers belong to the halo exchange
+        if (lo != 3) { a[0] = g0; a[stride] = g1; }
+        if (hi != 3) { a[(long long)(n + 2) * stride] = g2; a[(long long)(n + 3) * stride] = g3; }
     }
 }
 
@@ -285,11 +286,11 @@ template <int STAGE, int NDIM>
 __global__ void __launch_bounds__(128)
 stage_simple_kernel(Grid g, const double *__restrict__ Uin, const double *Uold, double *Uout,
                     double dt_over_dx, const StepScalars *__restrict__ dev_dt, double dx,
-                    StepScalars *__restrict__ red)
+                    StepScalars *__restrict__ red, int kz0)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = blockIdx.z;
+    const int k = blockIdx.z + kz0;
     double s = 0.0;
     int bad = 0;
     if (i < g.nx && j < g.ny) {
@@ -326,6 +327,31 @@ stage_simple_kernel(Grid g, const double *__restrict__ Uin, const double *Uold, 
             s = cell_signal_speed(un[0], un[1], un[2], un[3], un[4], g.gamma, g.gm1, bad);
     }
     if (STAGE == 2 && red) block_max_to_global(s, bad, &red->smax_bits, &red->flag);
+}
+
+// ------------------------------------------------------------------------------------------
+// Slab decomposition along z (the paper's domain decomposition): the two
+// active planes next to an interface go to the neighbouring slab's two ghost planes after every
+// substep.  MODE 0: padded planes K0, K0+1 -> packed buffer [5][2][ny][nx] (send side);
+// MODE 1: packed buffer -> padded planes (receive side); MODE 2: padded planes K0, K0+1 of this
+// slab -> padded planes Kd, Kd+1 of the neighbour's state `peer` (same nx, ny, pitch), i.e. the
+// exchange as direct peer stores -- over NVLink when `peer` lives on another GPU.
+// ------------------------------------------------------------------------------------------
+template <int MODE>
+__global__ void halo_kernel(Grid g, double *U, double *other, int K0, int Kd, long long peer_sv)
+{
+    const long long per_var = 2ll * g.ny * g.nx, total = NVAR * per_var;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total;
+         t += (long long)gridDim.x * blockDim.x) {
+        const int v = (int)(t / per_var);
+        const long long r = t % per_var;
+        const int i = (int)(r % g.nx);
+        const int j = (int)((r / g.nx) % g.ny), l = (int)(r / ((long long)g.nx * g.ny));
+        const long long c = v * g.sv + cell(g, i + NG, j + g.oy, K0 + l);
+        if (MODE == 0) other[t] = U[c];
+        else if (MODE == 1) U[c] = other[t];
+        else other[v * peer_sv + cell(g, i + NG, j + g.oy, Kd + l)] = U[c];
+    }
 }
 
 // ------------------------------------------------------------------------------------------

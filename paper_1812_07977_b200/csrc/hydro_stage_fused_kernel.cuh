@@ -12,6 +12,7 @@ struct FusedArgs {
     double dx;
     StepScalars *red;       // stage 2: max-signal-speed accumulator + sticky flag (or nullptr)
     int lz;                 // planes per z-chunk
+    int zc0;                // first z-chunk of this launch (a launch may cover a range of chunks)
     int inbc;               // bit a: the boundary rule of axis a is applied by this kernel (ghost layers of
                             // that axis are never read from memory); 0: all ghosts come from memory
 };
@@ -23,8 +24,9 @@ struct FusedArgs {
 // Branch-free: the boundary kinds are uniform, the selects cost a handful of integer instructions.
 __device__ __forceinline__ int bc_source(int i, int n, int lo, int hi, int cmin, int cmax, bool &flip)
 {
-    const int below = lo == 0 ? 0 : (lo == 1 ? -1 - i : i + n);
-    const int above = hi == 0 ? n - 1 : (hi == 1 ? 2 * n - 1 - i : i - n);
+    // kind 3 (neighbouring slab): the ghost layers exist in memory, written by the halo exchange
+    const int below = lo == 0 ? 0 : (lo == 1 ? -1 - i : (lo == 2 ? i + n : i));
+    const int above = hi == 0 ? n - 1 : (hi == 1 ? 2 * n - 1 - i : (hi == 2 ? i - n : i));
     flip = (i < 0 && lo == 1) || (i >= n && hi == 1);
     const int s = i < 0 ? below : (i >= n ? above : i);
     return min(max(s, cmin), cmax);
@@ -74,7 +76,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const Grid &g = a.g;
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;     // tile origin, active coordinates
-    const int k0 = blockIdx.z * a.lz;
+    const int k0 = (blockIdx.z + a.zc0) * a.lz;
     const int k1 = min(k0 + a.lz, g.nz);                      // chunk = active planes [k0, k1)
     const int nc = k1 - k0;                                   // cell planes; raw planes 0..nc+3
     const int nplanes = nc + 4;                               //   (raw plane p = active plane k0-2+p)
@@ -130,7 +132,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         tma::mbar_arrive_expect_tx(&bar[p % FNS], S::STAGE_BYTES);
         // z ghost planes are never materialised: request the source plane instead (clamp / mirror / wrap)
         bool fz;
-        const int K = (a.inbc & 4) ? bc_source(k0 + p - NG, g.nz, g.bc[4], g.bc[5], 0, g.nz - 1, fz) + NG : k0 + p;
+        const int K = (a.inbc & 4) ? bc_source(k0 + p - NG, g.nz, g.bc[4], g.bc[5], -NG, g.nz + NG - 1, fz) + NG : k0 + p;
         tma::load_4d(sm + S::OFF_RING + (p % FNS) * S::STAGE, &umap, i0, j0, K, 0, &bar[p % FNS]);
     };
     if (t == 0)

@@ -31,20 +31,35 @@ inline void fused_geometry(FusedPlan &p, const Grid &g, int ty, int lz)
     p.grid = dim3((g.nx + FTX - 1) / FTX, (g.ny + ty - 1) / ty, (g.nz + p.lz - 1) / p.lz);
 }
 
-// Planes per chunk: fill whole waves of (SMs x resident blocks) as evenly as possible while
-// keeping the four extra planes a chunk streams (two below, two above) a small overhead.
-inline int fused_choose_lz(const Grid &g, int ty, int nsm, int per_sm)
+// Launch geometry.  A block streams (l + 4) planes for l computed ones, but the four warm-up planes
+// only cost primitives and z-slopes, so with the block prologue a chunk of l planes takes about
+// (l + 2) plane times; blocks are handed to the SMs in waves of (SMs x resident blocks).  Measured on
+// B200 (tiling sweep): the best geometry is the one that fills whole waves,
+// short chunks are cheap, 32 x 16 tiles (one block per SM) beat 32 x 8 tiles (two per SM) at equal
+// wave count because they carry half the halo work, and a lone 32 x 8 block on an SM runs about 1.5
+// times faster than when it shares the SM (tiny grids: more, smaller blocks win).
+inline double fused_cost(const Grid &g, int ty, int l, int nsm)
 {
     const long long tiles = (long long)((g.nx + FTX - 1) / FTX) * ((g.ny + ty - 1) / ty);
+    const long long blocks = tiles * ((g.nz + l - 1) / l);
+    const int per_sm = ty == 16 ? 1 : 2;
     const long long slots = (long long)nsm * per_sm;
+    const long long waves = (blocks + slots - 1) / slots;
+    double cost = (double)waves * (l + 2);
+    if (ty == 8 && blocks <= nsm) cost *= 0.65;              // one 8-warp block per SM
+    if (ty == 16) cost *= 0.92;                              // half the halo / edge work per cell
+    return cost;
+}
+
+inline int fused_choose_lz(const Grid &g, int ty, int nsm, double *cost_out = nullptr)
+{
     int best = g.nz;
     double best_cost = 1e300;
-    for (int l = g.nz < 4 ? g.nz : 4; l <= g.nz; ++l) {
-        const long long blocks = tiles * ((g.nz + l - 1) / l);
-        const long long waves = (blocks + slots - 1) / slots;
-        const double cost = (double)waves * (l + 4);          // time ~ waves x planes per block
+    for (int l = g.nz; l >= (g.nz < 2 ? g.nz : 2); --l) {       // ties: the longer chunk (fewer blocks)
+        const double cost = fused_cost(g, ty, l, nsm);
         if (cost < best_cost - 1e-9) { best_cost = cost; best = l; }
     }
+    if (cost_out) *cost_out = best_cost;
     return best;
 }
 
@@ -61,12 +76,11 @@ inline cudaError_t plan_stage_fused(FusedPlan &p, const Grid &g, const double *A
     int nsm = 148, dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess)
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    // 32 x 16 tiles (one 512-thread block per SM) carry half the per-warp halo / edge work of 32 x 8
-    // tiles (two 256-thread blocks per SM) and win on large grids (256^3: 1.615 vs 1.636 ms per
-    // step); small grids need the finer tiling to fill the machine
-    int ty = g.ny >= 128 ? 16 : 8;
+    double c8, c16;
+    const int l8 = fused_choose_lz(g, 8, nsm, &c8), l16 = fused_choose_lz(g, 16, nsm, &c16);
+    int ty = c16 <= c8 ? 16 : 8;
     if (ty_req) ty = ty_req == 16 ? 16 : 8;
-    int lz = fused_choose_lz(g, ty, nsm, ty == 16 ? 1 : 2);
+    int lz = ty == 16 ? l16 : l8;
     if (lz_req > 0) lz = lz_req;
     fused_geometry(p, g, ty, lz);
     p.base[0] = A; p.base[1] = B;
@@ -82,21 +96,24 @@ template <int STAGE>
 inline cudaError_t launch_stage_fused(const FusedPlan &p, const Grid &g, const double *in,
                                       const double *old, double *out, double r,
                                       const StepScalars *dev_dt, double dx, StepScalars *red,
-                                      int inbc, cudaStream_t stream)
+                                      int inbc, cudaStream_t stream, int zc0 = 0, int nzc = -1)
 {
     if (!p.ready) return cudaErrorNotReady;
     const int b = in == p.base[0] ? 0 : 1;
     if (in != p.base[b]) return cudaErrorInvalidValue;
     FusedArgs a;
     a.g = g; a.Uold = old; a.Uout = out; a.dt_over_dx = r; a.dev_dt = dev_dt; a.dx = dx;
-    a.red = red; a.lz = p.lz; a.inbc = inbc;
+    a.red = red; a.lz = p.lz; a.inbc = inbc; a.zc0 = zc0;
+    dim3 grid = p.grid;
+    if (nzc >= 0) grid.z = (unsigned)nzc;                     // a range of z-chunks (slab runs: interface chunks first)
+    if (grid.z == 0) return cudaSuccess;
     const bool aniso = g.ry != 1.0 || g.rz != 1.0;            // non-cubic cells: two more DMUL per variable
     if (p.ty == 16) {
-        if (aniso) stage_fused_kernel<STAGE, 16, 1, true><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
-        else       stage_fused_kernel<STAGE, 16, 1, false><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
+        if (aniso) stage_fused_kernel<STAGE, 16, 1, true><<<grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
+        else       stage_fused_kernel<STAGE, 16, 1, false><<<grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
     } else {
-        if (aniso) stage_fused_kernel<STAGE, 8, 2, true><<<p.grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
-        else       stage_fused_kernel<STAGE, 8, 2, false><<<p.grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
+        if (aniso) stage_fused_kernel<STAGE, 8, 2, true><<<grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
+        else       stage_fused_kernel<STAGE, 8, 2, false><<<grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
     }
     return cudaGetLastError();
 }
