@@ -137,6 +137,30 @@ int hydro_set_allocator(void *(*alloc)(size_t bytes, void *stream), void (*relea
  * theta or the kernel variant changes).  The benchmark path (Algorithm 1's loop body without the
  * host-side ComputeTimeStep of Algorithm 2). */
 int hydro_run_steps(hydro_t *h, long long n);
+/* ---- host mirror with explicit, selective, overlapped transfers -------------------------------
+ * The paper's StorageForm keeps a host copy of the device storage and moves "all the selected fields
+ * ... en masse with a single call.  Alternatively, individual fields can be specified",
+ * from page-locked host memory for 1.7-2.0x faster transfers.  Same here, with
+ * the transfers off the compute stream:
+ * hydro_host_alloc: a pinned host buffer of one packed state U[5][nz][ny][nx], owned by the handle
+ *   (freed by hydro_destroy).  Any pinned or pageable host pointer works with the calls below; pinned
+ *   memory is what makes them asynchronous.
+ * hydro_update_device(h, fields, U_host): field v (bit v of `fields`: 1 rho, 2 m_x, 4 m_y, 8 m_z,
+ *   16 E) of the device state <- U_host, host-to-device on the handle's copy-in stream; work already
+ *   enqueued on the compute stream keeps running during the transfer, work enqueued afterwards sees
+ *   the new fields.  Keeps the clock (unlike hydro_set_state); the first update of a handle must bring
+ *   all five fields.
+ * hydro_update_host(h, fields, U_host): U_host <- selected fields of the state as of the work
+ *   enqueued so far: a device-side snapshot on the compute stream, then device-to-host on the copy-out
+ *   stream, so steps enqueued next overlap the transfer (and a following hydro_update_device's
+ *   transfer runs concurrently in the other direction).  U_host is valid after hydro_transfer_sync.
+ * hydro_transfer_sync: wait for the outstanding transfers of both directions.
+ * HYDRO_ERR_ARG for an empty or unknown field mask. */
+int hydro_host_alloc(hydro_t *h, double **U_host);
+int hydro_update_device(hydro_t *h, unsigned fields, const double *U_host);
+int hydro_update_host(hydro_t *h, unsigned fields, double *U_host);
+int hydro_transfer_sync(hydro_t *h);
+
 /* ---- domain decomposition into z-slabs ----------------------------------------------------
  * The paper runs the problem decomposed over MPI ranks, one GPU each, 256^3 cells per rank, with a
  * ghost exchange after every Runge-Kutta substep and a reduction of the time step every step

@@ -23,7 +23,8 @@ SYMBOLS = ["hydro_create", "hydro_create_nd", "hydro_set_state", "hydro_cfl_dt",
            "hydro_set_tiling", "hydro_get_tiling", "hydro_set_graph_replay",
            "hydro_create_slab", "hydro_substep", "hydro_halo_count", "hydro_halo_pack",
            "hydro_halo_unpack", "hydro_halo_push", "hydro_state_base", "hydro_smax_device",
-           "hydro_reduce_smax",
+           "hydro_reduce_smax", "hydro_host_alloc", "hydro_update_device", "hydro_update_host",
+           "hydro_transfer_sync",
            "hydro_set_profiling", "hydro_get_kernel_time", "hydro_launch_count",
            "hydro_is_verification_build", "hydro_last_error"]
 
@@ -89,6 +90,10 @@ def load_library(verify=False):
     L.hydro_state_base.argtypes = [vp, C.c_int, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.hydro_smax_device.argtypes = [vp, C.POINTER(vp)]
     L.hydro_reduce_smax.argtypes = [vp]
+    L.hydro_host_alloc.argtypes = [vp, C.POINTER(vp)]
+    L.hydro_update_device.argtypes = [vp, C.c_uint, vp]
+    L.hydro_update_host.argtypes = [vp, C.c_uint, vp]
+    L.hydro_transfer_sync.argtypes = [vp]
     L.hydro_set_profiling.argtypes = [vp, C.c_int]
     L.hydro_get_kernel_time.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_longlong)]
     L.hydro_launch_count.restype = C.c_longlong
@@ -292,6 +297,27 @@ class Hydro:
 
     def launch_count(self):
         return self._L.hydro_launch_count()
+
+    # ---- host mirror: selected fields, transfers overlapped with compute ----
+    def host_alloc(self):
+        """A pinned host array of one packed state, owned by the handle (numpy view)."""
+        p = C.c_void_p()
+        self._chk(self._L.hydro_host_alloc(self._h, C.byref(p)), "hydro_host_alloc")
+        n = int(np.prod(self.shape))
+        return np.ctypeslib.as_array(C.cast(p, _dp), shape=(n,)).reshape(self.shape)
+
+    def update_device(self, U_host, fields=31):
+        p, keep, on_device = _as_ptr(U_host, self.shape)
+        assert not on_device
+        self._chk(self._L.hydro_update_device(self._h, fields, p), "hydro_update_device")
+
+    def update_host(self, U_host, fields=31):
+        p, keep, on_device = _as_ptr(U_host, self.shape, writable=True)
+        assert not on_device
+        self._chk(self._L.hydro_update_host(self._h, fields, p), "hydro_update_host")
+
+    def transfer_sync(self):
+        self._chk(self._L.hydro_transfer_sync(self._h), "hydro_transfer_sync")
 
     # ---- z-slab decomposition (driver: paper_1812_07977_b200/slab.py) ----
     def substep(self, stage, dt=0.0, part=0):

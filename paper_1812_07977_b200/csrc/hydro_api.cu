@@ -72,6 +72,12 @@ struct hydro {
     // hydro_run_steps / hydro_evolve; rebuilt when anything baked into the launches changes
     cudaGraphExec_t step_graph = nullptr;
     int graph_kernels = 0;          // kernels per replay (for hydro_launch_count)
+    // host mirror (hydro_host_alloc / hydro_update_device / hydro_update_host): pinned host buffers
+    // owned by the handle, device staging buffers in the packed layout, one copy stream per direction
+    std::vector<double *> host_bufs;
+    double *stage_in = nullptr, *stage_out = nullptr;
+    cudaStream_t cin = nullptr, cout = nullptr;
+    cudaEvent_t ev_in_done = nullptr, ev_unpacked = nullptr, ev_packed = nullptr, ev_out_done = nullptr;
     // measurement hooks (hydro_set_profiling)
     bool profiling = false;
     struct Span { int which; cudaEvent_t a, b; };
@@ -270,8 +276,8 @@ int copy_state(hydro *h, double *padded, double *packed, bool to_padded)
         const long long nact = (long long)g.nx * g.ny * g.nz;
         long long blocks = (nact + 255) / 256;
         if (blocks > 148 * 16) blocks = 148 * 16;
-        if (to_padded) repack_kernel<true><<<(unsigned)blocks, 256, 0, h->stream>>>(g, padded, packed);
-        else repack_kernel<false><<<(unsigned)blocks, 256, 0, h->stream>>>(g, padded, packed);
+        if (to_padded) repack_kernel<true><<<(unsigned)blocks, 256, 0, h->stream>>>(g, padded, packed, 31u);
+        else repack_kernel<false><<<(unsigned)blocks, 256, 0, h->stream>>>(g, padded, packed, 31u);
         LAUNCH_CHECK("repack");
         return HYDRO_OK;
     }
@@ -483,6 +489,13 @@ int hydro_destroy(hydro_t *h)
     drop_graph(h);
     for (auto &s : h->spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
     for (auto e : h->pool) cudaEventDestroy(e);
+    if (h->cin) { cudaStreamSynchronize(h->cin); cudaStreamDestroy(h->cin); }
+    if (h->cout) { cudaStreamSynchronize(h->cout); cudaStreamDestroy(h->cout); }
+    for (cudaEvent_t e : { h->ev_in_done, h->ev_unpacked, h->ev_packed, h->ev_out_done })
+        if (e) cudaEventDestroy(e);
+    for (double *p : h->host_bufs) cudaFreeHost(p);
+    if (h->stage_in) cudaFree(h->stage_in);
+    if (h->stage_out) cudaFree(h->stage_out);
     dev_free(h, h->block);
     if (h->scal) cudaFree(h->scal);
     if (h->scal_host) cudaFreeHost(h->scal_host);
@@ -694,6 +707,111 @@ int hydro_evolve(hydro_t *h, double t_final, long long *nsteps)
     h->step += h->scal_host->steps;
     h->t_on_device = false;
     if (nsteps) *nsteps = h->scal_host->steps;
+    return HYDRO_OK;
+}
+
+// ---- host mirror (the paper's StorageForm: PAPER.md:62, 359-363) ----
+
+namespace {
+int mirror_setup(hydro *h)
+{
+    if (h->cin) return HYDRO_OK;
+    CUDA_TRY(cudaStreamCreateWithFlags(&h->cin, cudaStreamNonBlocking));
+    CUDA_TRY(cudaStreamCreateWithFlags(&h->cout, cudaStreamNonBlocking));
+    for (cudaEvent_t *e : { &h->ev_in_done, &h->ev_unpacked, &h->ev_packed, &h->ev_out_done })
+        CUDA_TRY(cudaEventCreateWithFlags(e, cudaEventDisableTiming));
+    return HYDRO_OK;
+}
+size_t packed_doubles(const hydro *h) { return (size_t)NVAR * h->g.nx * h->g.ny * h->g.nz; }
+// copies the selected fields (runs of adjacent fields as one transfer)
+int copy_fields(double *dst, const double *src, size_t n, unsigned fields, cudaMemcpyKind kind, cudaStream_t st)
+{
+    for (int v = 0; v < NVAR;) {
+        if (!(fields >> v & 1u)) { ++v; continue; }
+        int w = v;
+        while (w + 1 < NVAR && (fields >> (w + 1) & 1u)) ++w;
+        CUDA_TRY(cudaMemcpyAsync(dst + v * n, src + v * n, (size_t)(w - v + 1) * n * sizeof(double), kind, st));
+        v = w + 1;
+    }
+    return HYDRO_OK;
+}
+unsigned repack_blocks(const hydro *h)
+{
+    const long long nact = (long long)h->g.nx * h->g.ny * h->g.nz;
+    long long b = (nact + 255) / 256;
+    return (unsigned)(b > 148 * 16 ? 148 * 16 : b);
+}
+}  // namespace
+
+int hydro_host_alloc(hydro_t *h, double **U_host)
+{
+    if (!h || !U_host) return fail(HYDRO_ERR_ARG, "host_alloc: NULL argument%s%s");
+    double *p = nullptr;
+    cudaError_t e = cudaHostAlloc((void **)&p, packed_doubles(h) * sizeof(double), cudaHostAllocDefault);
+    if (e != cudaSuccess) { cudaGetLastError(); return fail(HYDRO_ERR_ALLOC, "host_alloc: %s%s", cudaGetErrorString(e)); }
+    h->host_bufs.push_back(p);
+    *U_host = p;
+    return HYDRO_OK;
+}
+
+int hydro_update_device(hydro_t *h, unsigned fields, const double *U_host)
+{
+    if (!h || !U_host || !(fields & 31u) || (fields & ~31u)) return fail(HYDRO_ERR_ARG, "update_device: bad argument%s%s");
+    if (!h->have_state && (fields & 31u) != 31u)
+        return fail(HYDRO_ERR_NOSTATE, "update_device: the first update must bring all five fields%s%s");
+    int rc = mirror_setup(h);
+    if (rc) return rc;
+    const size_t n = (size_t)h->g.nx * h->g.ny * h->g.nz;
+    if (!h->stage_in) {
+        cudaError_t e = cudaMalloc((void **)&h->stage_in, NVAR * n * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(HYDRO_ERR_ALLOC, "update_device: %s%s", cudaGetErrorString(e)); }
+        CUDA_TRY(cudaEventRecord(h->ev_unpacked, h->stream));
+    }
+    // copy stream: after the previous unpack has read the staging buffer; then H2D of the selected fields
+    CUDA_TRY(cudaStreamWaitEvent(h->cin, h->ev_unpacked, 0));
+    if ((rc = copy_fields(h->stage_in, U_host, n, fields, cudaMemcpyHostToDevice, h->cin))) return rc;
+    CUDA_TRY(cudaEventRecord(h->ev_in_done, h->cin));
+    // compute stream: whatever was enqueued before keeps running during the transfer; the unpack
+    // (and everything enqueued after this call) waits for it
+    CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_in_done, 0));
+    if (h->t_on_device && (rc = read_scalars(h))) return rc;
+    repack_kernel<true><<<repack_blocks(h), 256, 0, h->stream>>>(h->g, h->A, h->stage_in, fields);
+    LAUNCH_CHECK("unpack");
+    CUDA_TRY(cudaEventRecord(h->ev_unpacked, h->stream));
+    CUDA_TRY(cudaMemsetAsync(&h->scal->flag, 0, sizeof(int), h->stream));
+    h->have_state = true; h->smax_valid = false;
+    return HYDRO_OK;
+}
+
+int hydro_update_host(hydro_t *h, unsigned fields, double *U_host)
+{
+    if (!h || !U_host || !(fields & 31u) || (fields & ~31u)) return fail(HYDRO_ERR_ARG, "update_host: bad argument%s%s");
+    if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "update_host before any state%s%s");
+    int rc = mirror_setup(h);
+    if (rc) return rc;
+    const size_t n = (size_t)h->g.nx * h->g.ny * h->g.nz;
+    if (!h->stage_out) {
+        cudaError_t e = cudaMalloc((void **)&h->stage_out, NVAR * n * sizeof(double));
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(HYDRO_ERR_ALLOC, "update_host: %s%s", cudaGetErrorString(e)); }
+        CUDA_TRY(cudaEventRecord(h->ev_out_done, h->cout));
+    }
+    // compute stream: snapshot of the selected fields into the packed staging buffer (HBM to HBM), after
+    // the previous device-to-host transfer has drained it; the steps enqueued next do not wait
+    CUDA_TRY(cudaStreamWaitEvent(h->stream, h->ev_out_done, 0));
+    repack_kernel<false><<<repack_blocks(h), 256, 0, h->stream>>>(h->g, h->A, h->stage_out, fields);
+    LAUNCH_CHECK("pack");
+    CUDA_TRY(cudaEventRecord(h->ev_packed, h->stream));
+    CUDA_TRY(cudaStreamWaitEvent(h->cout, h->ev_packed, 0));
+    if ((rc = copy_fields(U_host, h->stage_out, n, fields, cudaMemcpyDeviceToHost, h->cout))) return rc;
+    CUDA_TRY(cudaEventRecord(h->ev_out_done, h->cout));
+    return HYDRO_OK;
+}
+
+int hydro_transfer_sync(hydro_t *h)
+{
+    if (!h) return fail(HYDRO_ERR_ARG, "transfer_sync: NULL handle%s%s");
+    if (h->cin) CUDA_TRY(cudaStreamSynchronize(h->cin));
+    if (h->cout) CUDA_TRY(cudaStreamSynchronize(h->cout));
     return HYDRO_OK;
 }
 

@@ -359,7 +359,7 @@ __global__ void halo_kernel(Grid g, double *U, double *other, int K0, int Kd, lo
 // host pointers go through cudaMemcpy3D in the API layer).
 // ------------------------------------------------------------------------------------------
 template <bool TO_PADDED>
-__global__ void repack_kernel(Grid g, double *padded, double *packed)
+__global__ void repack_kernel(Grid g, double *padded, double *packed, unsigned fields)
 {
     const long long nact = (long long)g.nx * g.ny * g.nz;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nact;
@@ -370,6 +370,7 @@ __global__ void repack_kernel(Grid g, double *padded, double *packed)
         const long long c = cell0(g, i, j, k);
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) {
+            if (!(fields >> v & 1u)) continue;               // selected fields only
             if (TO_PADDED) padded[v * g.sv + c] = packed[v * nact + t];
             else packed[v * nact + t] = padded[v * g.sv + c];
         }
