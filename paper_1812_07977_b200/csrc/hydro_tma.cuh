@@ -47,18 +47,6 @@ __device__ __forceinline__ void mbar_arrive(uint64_t *bar)
 
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
-#ifdef HYD_WAITHINT
-    asm volatile(
-        "{\n"
-        ".reg .pred P1;\n"
-        "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
-        "@P1 bra DONE;\n"
-        "bra LAB_WAIT;\n"
-        "DONE:\n"
-        "}" ::"r"(smem_u32(bar)), "r"(parity), "r"((uint32_t)HYD_WAITHINT)
-        : "memory");
-#else
     asm volatile(
         "{\n"
         ".reg .pred P1;\n"
@@ -69,7 +57,6 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "DONE:\n"
         "}" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
-#endif
 }
 
 // one rank-4 box: coordinates (c0 fastest) -> shared memory at dst, completion on bar
