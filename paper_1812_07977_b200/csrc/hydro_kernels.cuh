@@ -2,7 +2,7 @@
 // (A2-A7), CFL reduction (A8), time-step bookkeeping.  See DESIGN.md section 5 for the layout and
 // section 6 for each kernel's roofline.
 #pragma once
-#include "hydro_math.cuh"
+#include "hydro_faces.cuh"
 
 namespace hyd {
 
@@ -238,48 +238,28 @@ cfl_reduce_kernel(Grid g, const double *__restrict__ U, unsigned long long *smax
 // Same arithmetic as the fused kernel; kept as the bring-up and cross-check implementation.
 // STAGE 1: out = U0 + dU(U0).   STAGE 2: out = 0.5*((U0 + U1) + dU(U1)) (+ fused CFL max).
 // ------------------------------------------------------------------------------------------
-template <int D>
-__device__ __forceinline__ void load_prim_line(const Grid &g, const double *__restrict__ U,
-                                               long long c, long long stride, double W[5][5])
-{
-    // W[o][.] = primitives of the cell at offset o-2 along D, in (rho, n, t1, t2, p) order
-#pragma unroll
-    for (int o = 0; o < 5; ++o) {
-        const long long cc = c + (o - 2) * stride;
-        const Prim w = primitive(__ldg(U + cc), __ldg(U + g.sv + cc), __ldg(U + 2 * g.sv + cc),
-                                 __ldg(U + 3 * g.sv + cc), __ldg(U + 4 * g.sv + cc), g.gm1);
-        const double v[3] = { w.vx, w.vy, w.vz };
-        W[o][0] = w.rho; W[o][1] = v[D]; W[o][2] = v[(D + 1) % 3]; W[o][3] = v[(D + 2) % 3];
-        W[o][4] = w.p;
-    }
-}
-
+// flux difference F(i+1/2) - F(i-1/2) along D of one cell, (rho, mx, my, mz, E) order
 template <int D>
 __device__ __forceinline__ void flux_difference(const Grid &g, const double *__restrict__ U,
                                                 long long c, long long stride, double dF[5])
 {
-    double W[5][5];
-    load_prim_line<D>(g, U, c, stride, W);
-    double Lm[5], Rm[5], Lp[5], Rp[5];     // faces i-1/2 and i+1/2
+    double W[5][5];                         // primitives (rho, vx, vy, vz, p) of cells i-2 .. i+2 along D
 #pragma unroll
-    for (int v = 0; v < 5; ++v) {
-        const double sm = minmod(g.theta, W[1][v] - W[0][v], W[2][v] - W[1][v]);
-        const double s0 = minmod(g.theta, W[2][v] - W[1][v], W[3][v] - W[2][v]);
-        const double sp = minmod(g.theta, W[3][v] - W[2][v], W[4][v] - W[3][v]);
-        Lm[v] = W[1][v] + 0.5 * sm;      // outer(i-1)
-        Rm[v] = W[2][v] - 0.5 * s0;      // inner(i)
-        Lp[v] = W[2][v] + 0.5 * s0;      // outer(i)
-        Rp[v] = W[3][v] - 0.5 * sp;      // inner(i+1)
+    for (int o = 0; o < 5; ++o) {
+        const long long cc = c + (o - 2) * stride;
+        const double Uc[5] = { __ldg(U + cc), __ldg(U + g.sv + cc), __ldg(U + 2 * g.sv + cc),
+                               __ldg(U + 3 * g.sv + cc), __ldg(U + 4 * g.sv + cc) };
+        HYD_PRIM5(Uc, g.gm1, W[o]);
     }
+    double Im[5], Om[5], I0[5], O0[5], Ip[5], Op[5];    // inner / outer face values of cells i-1, i, i+1
+    HYD_LIMITED_FACES(g.theta, W[0], W[1], W[2], Im, Om);
+    HYD_LIMITED_FACES(g.theta, W[1], W[2], W[3], I0, O0);
+    HYD_LIMITED_FACES(g.theta, W[2], W[3], W[4], Ip, Op);
     double Fm[5], Fp[5];
-    hll_flux(Lm, Rm, g.gamma, g.igm1, Fm);
-    hll_flux(Lp, Rp, g.gamma, g.igm1, Fp);
-    // (rho, n, t1, t2, E) -> (rho, mx, my, mz, E)
-    dF[0] = Fp[0] - Fm[0];
-    dF[1 + D] = Fp[1] - Fm[1];
-    dF[1 + (D + 1) % 3] = Fp[2] - Fm[2];
-    dF[1 + (D + 2) % 3] = Fp[3] - Fm[3];
-    dF[4] = Fp[4] - Fm[4];
+    face_flux<D>(Om, I0, g.gamma, g.igm1, Fm);          // face i-1/2: left = outer(i-1), right = inner(i)
+    face_flux<D>(O0, Ip, g.gamma, g.igm1, Fp);          // face i+1/2
+#pragma unroll
+    for (int v = 0; v < 5; ++v) dF[v] = Fp[v] - Fm[v];
 }
 
 template <int STAGE, int NDIM>
@@ -323,8 +303,14 @@ stage_simple_kernel(Grid g, const double *__restrict__ Uin, const double *Uold, 
             }
             Uout[v * g.sv + c] = un[v];
         }
-        if (STAGE == 2 && red)
+        if (STAGE == 2 && red) {
+#ifdef HYDRO_VERIFY
             s = cell_signal_speed(un[0], un[1], un[2], un[3], un[4], g.gamma, g.gm1, bad);
+#else
+            s = fast::signal_speed(un, g.gamma, g.gm1, bad);
+            if (!(s <= 1.79769313486231570e308)) { bad = 1; s = 0.0; }      // inf or NaN
+#endif
+        }
     }
     if (STAGE == 2 && red) block_max_to_global(s, bad, &red->smax_bits, &red->flag);
 }

@@ -247,6 +247,13 @@ class HydroEngine:
     def stream(self):
         return self.h.torch_stream
 
+    def reduce_smax(self):
+        self.h.reduce_smax()
+
+    def smax_tensor(self):
+        """The running maximum of the signal speed on the device, as a 1-element tensor (no copy)."""
+        return self.torch.as_tensor(_DevPtr(self.h.smax_device(), 1), device="cuda")
+
 
 class SlabRank:
     """One slab per process; `dist` is torch.distributed (initialised).  NCCL: the packed device
@@ -331,7 +338,25 @@ class SlabRank:
         dxs = self.dx / float(s.item())
         return c3 * dxs
 
+    def run_steps(self, n):
+        """n steps with the time step kept on the devices: the running maximum is all-reduced in place
+        (NCCL, ordered on the slab's stream) and every slab forms the same dt from it at the start of
+        substep 1.  Other backends fall back to the host-side reduction."""
+        if not self.device_comm:
+            for _ in range(n):
+                self.step(self.cfl_dt())
+            return
+        import torch
+        if self._first:
+            self.e.reduce_smax()
+        smax = self.e.smax_tensor()
+        for _ in range(n):
+            with torch.cuda.stream(self.e.stream()):
+                self.dist.all_reduce(smax, op=self.dist.ReduceOp.MAX)
+            self.step(0.0)
+
     def step(self, dt):
+        """dt > 0: host-supplied step; dt == 0: device-resident (run_steps)."""
         if self._first:
             self._start_exchange(0)
             self._first = False
