@@ -1,10 +1,6 @@
 // hydro_stage_fused_kernel.cuh -- body of the fused stage kernel (see hydro_stage_fused.cuh).
 #pragma once
 
-#ifndef HYD_WT
-#define HYD_WT 0
-#endif
-
 namespace hyd {
 
 struct FusedArgs {
@@ -283,11 +279,6 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             HYD_PRIM5(Un, gm1, Wn);
             HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
-#if HYD_WT == 1
-        if (PIPE && c + 1 < nc)
-            write_tile(sm + S::OFF_W + ((c + 1) & 1) * S::STAGE, Wb,
-                       sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE, (ty + c + 1) & (TY - 1));
-#endif
         tma::mbar_wait(barO, par);
         if (PIPE) __syncwarp();                               // the warp's own outer x values are in place
         // every warp is past P4 of cell plane c-1: raw plane c+1 is dead, refill its stage
@@ -296,11 +287,9 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         double Fxl[5], Fyl[5];
         // PIPE: primitive tile of cell plane c+1 into the other buffer (free since wait_F(c-1), read
         // after wait_F(c)); own cell = W(c+1) = Wb, halo cells from raw plane c+3
-#if HYD_WT != 1
         if (PIPE && c + 1 < nc)
             write_tile(sm + S::OFF_W + ((c + 1) & 1) * S::STAGE, Wb,
                        sm + S::OFF_RING + ((c + 3) % FNS) * S::STAGE, (ty + c + 1) & (TY - 1));
-#endif
         {
             double L[5];
 #pragma unroll
