@@ -209,13 +209,14 @@ int hydro_get_padded(hydro_t *h, double *Upad);
 /* Tuning hooks of the fused stage kernel (tests and measurement; defaults are chosen per grid).
  * hydro_set_tiling: tile_rows = 8 | 16 (rows of 32 cells per block; 0 = chosen by the library),
  * planes_per_chunk = z-planes a block marches over (0 = chosen so that the blocks fill whole waves
- * of the SMs).  hydro_get_tiling reports the geometry in use and the number of blocks per stage
+ * of the SMs; for a 2D run: 32 x 16 tiles a block walks down y).  hydro_get_tiling reports the geometry in use and the number of blocks per stage
  * launch (any out-pointer may be NULL).  hydro_set_graph_replay(h, 0) makes hydro_run_steps /
  * hydro_evolve enqueue plain launches instead of replaying the captured one-step CUDA graph. */
 int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk);
 int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long long *blocks);
 int hydro_set_graph_replay(hydro_t *h, int enable);
-/* Select the stage-kernel implementation: 0 = reference-structured simple kernel (one thread per
+/* Select the stage-kernel implementation (2D and 3D runs; a 1D run always uses 0):
+ * 0 = reference-structured simple kernel (one thread per
  * cell, everything recomputed, ghost layers filled in memory before each substep); 1 = fused tiled
  * kernel with the boundary rules applied in the kernel (default: ghost layers are written to memory
  * only for periodic x / y faces, and not at all otherwise -- three launches per step); 2 = the same

@@ -5,6 +5,7 @@
 #include "../../include/hydro.h"
 #include "hydro_kernels.cuh"
 #include "hydro_stage_fused.cuh"
+#include "hydro_stage_fused2d.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -155,8 +156,8 @@ int is_device_pointer(const void *p, bool *on_device)
 // need the fill kernel; variant 2 (fused kernel reading memory ghosts) and the simple kernel need all.
 int fill_axes(const hydro *h)
 {
-    if (h->g.ndim < 3) return (1 << h->g.ndim) - 1;      // 1D / 2D runs: simple kernel, active axes only
-    if (h->variant != 1) return 7;
+    const int active = (1 << h->g.ndim) - 1;             // inactive axes have no ghost layers
+    if (h->g.ndim == 1 || h->variant != 1) return active;    // simple kernel / variant 2: ghosts from memory
     int axes = 0;
     if (h->g.bc[0] == HYDRO_BC_PERIODIC) axes |= 1;
     if (h->g.bc[2] == HYDRO_BC_PERIODIC) axes |= 2;
@@ -213,7 +214,7 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
     const StepScalars *dd = dev_dt ? h->scal : nullptr;
     StepScalars *red = reduce ? h->scal : nullptr;
     Scope sc(h, STAGE == 1 ? K_STAGE1 : K_STAGE2);
-    if (h->variant == 0 || g.ndim < 3) {      // (variants 1 and 2 are the fused kernel, 3D runs only)
+    if (h->variant == 0 || g.ndim == 1) {     // (variants 1 and 2 are the fused kernels of 2D / 3D runs)
         dim3 tb(32, 4, 1);
         if (g.ndim == 1) tb = dim3(128, 1, 1);
         dim3 gr((g.nx + tb.x - 1) / tb.x, (g.ny + tb.y - 1) / tb.y, ke - kb);
@@ -223,7 +224,13 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
         LAUNCH_CHECK("stage_simple");
         return HYDRO_OK;
     }
-    const int inbc = h->variant == 1 ? 7 & ~fill_axes(h) : 0;
+    const int inbc = h->variant == 1 ? ((1 << g.ndim) - 1) & ~fill_axes(h) : 0;
+    if (g.ndim == 2) {
+        cudaError_t e2 = launch_stage_fused2d<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (e2 != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused2d: %s%s", cudaGetErrorString(e2));
+        return HYDRO_OK;
+    }
     const int lz = h->plan.lz;
     cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream,
                                               kb / lz, (ke - kb + lz - 1) / lz);
@@ -445,7 +452,7 @@ int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, c
         if (a < ndim && d[a] < h->dmin) h->dmin = d[a];
     }
     g.ry = h->dx / h->dxyz[1]; g.rz = h->dx / h->dxyz[2];
-    if (ndim < 3) h->variant = 0;
+    if (ndim == 1) h->variant = 0;
     // +16 tail so vectorised / TMA reads that run a few doubles past the last row stay inside
     h->buf_doubles = (size_t)LEAD + (size_t)NVAR * g.sv + 16 + 2;
     h->buf_doubles = ((h->buf_doubles + 15) / 16) * 16;
@@ -460,6 +467,7 @@ int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, c
     if (e == cudaSuccess) e = cudaMemset(h->block, 0, 2 * h->buf_doubles * sizeof(double));
     if (e == cudaSuccess) e = cudaMemset(h->scal, 0, sizeof(StepScalars));
     if (e == cudaSuccess && ndim == 3) e = plan_stage_fused(h->plan, g, h->A, h->B);
+    if (e == cudaSuccess && ndim == 2) e = plan_stage_fused2d(h->plan, g, h->A, h->B);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();   // the memsets ran on the legacy stream; the handle's
                                                          // stream may be a non-blocking one
     if (e != cudaSuccess) {
@@ -532,8 +540,8 @@ int hydro_set_limiter_theta(hydro_t *h, double theta)
 int hydro_set_kernel_variant(hydro_t *h, int variant)
 {
     if (!h || variant < 0 || variant > 2) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0, 1 or 2%s%s");
-    if (h->g.ndim < 3 && variant != 0)
-        return fail(HYDRO_ERR_ARG, "set_kernel_variant: 1D / 2D runs use the simple kernel (variant 0)%s%s");
+    if (h->g.ndim == 1 && variant != 0)
+        return fail(HYDRO_ERR_ARG, "set_kernel_variant: 1D runs use the simple kernel (variant 0)%s%s");
     h->variant = variant;
     drop_graph(h);
     return HYDRO_OK;
@@ -552,11 +560,13 @@ int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk)
     if (!h) return fail(HYDRO_ERR_ARG, "set_tiling: NULL handle%s%s");
     if ((tile_rows != 0 && tile_rows != 8 && tile_rows != 16) || planes_per_chunk < 0)
         return fail(HYDRO_ERR_ARG, "set_tiling: tile_rows must be 0, 8 or 16 and planes_per_chunk >= 0%s%s");
-    if (h->g.ndim < 3) return fail(HYDRO_ERR_ARG, "set_tiling: the fused kernel runs 3D grids only%s%s");
+    if (h->g.ndim == 1 || (h->g.ndim == 2 && tile_rows == 8))
+        return fail(HYDRO_ERR_ARG, "set_tiling: 1D runs have no fused kernel; 2D runs use 32 x 16 tiles%s%s");
     CUDA_TRY(cudaStreamSynchronize(h->stream));
     drop_graph(h);
     h->ty_req = tile_rows; h->lz_req = planes_per_chunk;
-    cudaError_t e = plan_stage_fused(h->plan, h->g, h->A, h->B, h->ty_req, h->lz_req);
+    cudaError_t e = h->g.ndim == 2 ? plan_stage_fused2d(h->plan, h->g, h->A, h->B, h->lz_req)
+                                   : plan_stage_fused(h->plan, h->g, h->A, h->B, h->ty_req, h->lz_req);
     if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "set_tiling: %s%s", cudaGetErrorString(e));
     return HYDRO_OK;
 }

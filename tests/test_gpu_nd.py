@@ -35,6 +35,9 @@ CASES = [
     (2, (70, 37, 1), (0.02, 0.02, 1.0), (OUT, REF, PER, PER, OUT, OUT)),
     (2, (33, 5, 1), (0.1, 0.031, 1.0), (PER, PER, REF, OUT, OUT, OUT)),
     (2, (2, 2, 1), (0.1, 0.4, 1.0), (REF, REF, REF, REF, OUT, OUT)),
+    (2, (100, 130, 1), (0.01, 0.01, 1.0), (OUT, OUT, OUT, OUT, OUT, OUT)),   # fused 2D kernel: 4 x 9 tiles
+    (2, (45, 83, 1), (0.02, 0.013, 1.0), (REF, OUT, OUT, REF, OUT, OUT)),
+    (2, (64, 64, 1), (0.02, 0.02, 1.0), (PER, PER, PER, PER, OUT, OUT)),
     (3, (37, 21, 9), (0.1, 0.07, 0.23), (OUT, REF, PER, PER, REF, OUT)),     # fused kernel, non-cubic cells
     (3, (40, 18, 35), (0.05, 0.05, 0.011), (PER, PER, OUT, OUT, REF, REF)),
 ]
@@ -43,9 +46,11 @@ CASES = [
 @pytest.mark.parametrize("ndim,shape,dxyz,bc", CASES)
 def test_nd_runs_bit_identical_on_verification_build(ndim, shape, dxyz, bc):
     U = inputs.random_state(*shape, seed=sum(shape) + ndim, vamp=0.5)
-    variants = (1, 2, 0) if ndim == 3 else (None,)
+    variants = (1, 2, 0) if ndim >= 2 else (None,)
     for variant in variants:
         g, c = _pair(shape, ndim, dxyz, bc, variant=variant)
+        if ndim == 2 and variant == 2:
+            g.set_tiling(16, 2)                            # several chunks of two tile rows per column
         g.set_state(U); c.set_state(U)
         assert g.get_padded().shape == c.get_padded().shape
         for _ in range(3):
@@ -132,7 +137,11 @@ def test_create_nd_status_codes():
     with pytest.raises(HydroError):
         Hydro(8, 8, 1, 1.4, 0.1, (0,) * 6, ndim=2, dxyz=(0.1, -0.1, 0.1))
     g = Hydro(8, 8, 1, 1.4, 0.1, (0,) * 6, ndim=2, dxyz=(0.1, 0.2, 0.1))
+    g.set_kernel_variant(1); g.set_tiling(16, 4)
     with pytest.raises(HydroError):
-        g.set_kernel_variant(1)                            # fused kernel: 3D runs only
+        g.set_tiling(8, 4)                                 # 2D runs use 32 x 16 tiles
+    g = Hydro(8, 1, 1, 1.4, 0.1, (0,) * 6, ndim=1, dxyz=(0.1, 0.2, 0.1))
     with pytest.raises(HydroError):
-        g.set_tiling(8, 4)
+        g.set_kernel_variant(1)                            # 1D runs: simple kernel only
+    with pytest.raises(HydroError):
+        g.set_tiling(16, 4)
