@@ -63,6 +63,7 @@ struct hydro {
     bool have_state = false;
     bool smax_valid = false;        // scal->smax_bits holds max(|v|+c) of the current state
     bool t_on_device = false;       // run_steps advanced the device clock
+    bool ghosts_valid = false;      // periodic x / y ghost layers of A are current (fused kernel, variant 1)
     double t = 0.0;
     long long step = 0;
     int variant = 1;
@@ -150,18 +151,40 @@ int is_device_pointer(const void *p, bool *on_device)
     return HYDRO_OK;
 }
 
-// Which axes still get their ghost layers written to memory before a stage (GhostExchange,
-// PAPER.md:152, 172, 186).  The fused stage kernel applies outflow and reflecting rules itself and
-// serves every z ghost plane by remapping the TMA plane coordinate, so only periodic x / y faces
-// need the fill kernel; variant 2 (fused kernel reading memory ghosts) and the simple kernel need all.
-int fill_axes(const hydro *h)
+// Boundaries of the fused stage kernels (variant 1; GhostExchange).  Outflow
+// and reflecting rules are applied in the kernel and every z ghost plane is served by remapping the
+// TMA plane coordinate, so only periodic x / y faces need ghost layers in memory.  Those are either
+// kept current by the producer (wrap stores in the update; ghost_fill_kernel then runs once after the
+// state was set from outside, ensure_ghosts) or filled by ghost_fill_kernel before every stage.  The
+// first is one launch less per stage and wins up to 256^3 (64^3: 43 -> 39 us per step); on larger
+// grids the partial-sector stores of the x images cost more than the fill kernel (512^3: stage 2
+// +8 %), so those keep the fill.  Variant 2 (fused kernel, every ghost layer from memory) and the
+// simple kernel fill all active axes before every stage.
+int periodic_xy(const hydro *h)
 {
-    const int active = (1 << h->g.ndim) - 1;             // inactive axes have no ghost layers
-    if (h->g.ndim == 1 || h->variant != 1) return active;    // simple kernel / variant 2: ghosts from memory
     int axes = 0;
     if (h->g.bc[0] == HYDRO_BC_PERIODIC) axes |= 1;
-    if (h->g.bc[2] == HYDRO_BC_PERIODIC) axes |= 2;
+    if (h->g.ndim >= 2 && h->g.bc[2] == HYDRO_BC_PERIODIC) axes |= 2;
     return axes;
+}
+
+bool fused_run(const hydro *h) { return h->g.ndim >= 2 && h->variant == 1; }
+
+int wrap_axes(const hydro *h)      // periodic axes whose ghost layers the stage kernels maintain
+{
+    const long long cells = (long long)h->g.nx * h->g.ny * h->g.nz;
+    return fused_run(h) && cells <= (1ll << 25) ? periodic_xy(h) : 0;
+}
+
+int fill_axes(const hydro *h)      // axes ghost_fill_kernel fills before every stage
+{
+    if (!fused_run(h)) return (1 << h->g.ndim) - 1;       // inactive axes have no ghost layers
+    return periodic_xy(h) & ~wrap_axes(h);
+}
+
+int inkernel_axes(const hydro *h)  // axes whose boundary rule the fused kernels apply themselves
+{
+    return fused_run(h) ? ((1 << h->g.ndim) - 1) & ~periodic_xy(h) : 0;
 }
 
 int launch_ghost_fill(hydro *h, double *U, bool clear_smax, bool advance_dt = false, int axes = 7)
@@ -204,6 +227,17 @@ int launch_cfl_reduce(hydro *h)
 
 // One substep over the active planes [kb, ke) (whole grid: 0, nz).  The fused kernel works in
 // z-chunks of plan.lz planes, so kb and ke must be chunk boundaries (or nz).
+// After the state was set from outside, the periodic x / y ghost layers of A are filled once.
+int ensure_ghosts(hydro *h)
+{
+    if (h->ghosts_valid) return HYDRO_OK;
+    const int axes = wrap_axes(h);
+    int rc;
+    if (axes && (rc = launch_ghost_fill(h, h->A, false, false, axes))) return rc;
+    h->ghosts_valid = true;
+    return HYDRO_OK;
+}
+
 template <int STAGE>
 int launch_stage(hydro *h, const double *in, const double *old, double *out, double r,
                  bool dev_dt, bool reduce, int kb = 0, int ke = -1)
@@ -224,16 +258,17 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
         LAUNCH_CHECK("stage_simple");
         return HYDRO_OK;
     }
-    const int inbc = h->variant == 1 ? ((1 << g.ndim) - 1) & ~fill_axes(h) : 0;
+    const int inbc = inkernel_axes(h);
     if (g.ndim == 2) {
-        cudaError_t e2 = launch_stage_fused2d<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream);
+        cudaError_t e2 = launch_stage_fused2d<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, wrap_axes(h),
+                                                     h->stream);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e2 != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused2d: %s%s", cudaGetErrorString(e2));
         return HYDRO_OK;
     }
     const int lz = h->plan.lz;
-    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, h->stream,
-                                              kb / lz, (ke - kb + lz - 1) / lz);
+    cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, wrap_axes(h),
+                                              h->stream, kb / lz, (ke - kb + lz - 1) / lz);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused: %s%s", cudaGetErrorString(e));
     return HYDRO_OK;
@@ -246,13 +281,13 @@ int enqueue_step(hydro *h, double dt_host, bool dev_dt)
     int rc;
     const int axes = fill_axes(h);
     if (axes) {
-        // device dt: the first fill of the step also forms dt = (cfl/3) dx / smax and advances the
+        // (simple kernel, variant 2) device dt: the first fill of the step also forms dt = (cfl/3) dx / smax and advances the
         // clock; the second one clears the accumulator of the reduction fused into stage 2
         if ((rc = launch_ghost_fill(h, h->A, false, dev_dt, axes))) return rc;
         if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
         if ((rc = launch_ghost_fill(h, h->B, true, false, axes))) return rc;
     } else {
-        // every boundary is applied inside the stage kernels: three launches per step
+        // the stage kernels handle every boundary themselves: three launches per step
         if ((rc = launch_begin_step(h, dev_dt))) return rc;
         if ((rc = launch_stage<1>(h, h->A, nullptr, h->B, r, dev_dt, false))) return rc;
     }
@@ -318,6 +353,7 @@ void drop_graph(hydro *h)
 int enqueue_device_steps(hydro *h, long long n)
 {
     int rc;
+    if ((rc = ensure_ghosts(h))) return rc;                  // not part of the captured step
     const bool use_graph = h->stream != nullptr && !h->profiling && h->graph_replay;
     if (use_graph && !h->step_graph) {
         const long long before = g_launches.load();
@@ -543,6 +579,7 @@ int hydro_set_kernel_variant(hydro_t *h, int variant)
     if (h->g.ndim == 1 && variant != 0)
         return fail(HYDRO_ERR_ARG, "set_kernel_variant: 1D runs use the simple kernel (variant 0)%s%s");
     h->variant = variant;
+    h->ghosts_valid = false;
     drop_graph(h);
     return HYDRO_OK;
 }
@@ -589,6 +626,7 @@ int hydro_set_state(hydro_t *h, const double *U)
     CUDA_TRY(cudaStreamSynchronize(h->stream));   // host or device pointer: the caller may free or
                                                   // overwrite U on return (hydro.h)
     h->t = 0.0; h->step = 0; h->have_state = true; h->smax_valid = false; h->t_on_device = false;
+    h->ghosts_valid = false;
     return HYDRO_OK;
 }
 
@@ -657,6 +695,7 @@ int hydro_step(hydro_t *h, double dt)
     if (!h->have_state) return fail(HYDRO_ERR_NOSTATE, "step before set_state%s%s");
     int rc;
     if (h->t_on_device && (rc = read_scalars(h))) return rc;
+    if ((rc = ensure_ghosts(h))) return rc;
     if ((rc = enqueue_step(h, dt, false))) return rc;
     h->t = h->t + dt;
     h->step += 1;
@@ -789,7 +828,7 @@ int hydro_update_device(hydro_t *h, unsigned fields, const double *U_host)
     LAUNCH_CHECK("unpack");
     CUDA_TRY(cudaEventRecord(h->ev_unpacked, h->stream));
     CUDA_TRY(cudaMemsetAsync(&h->scal->flag, 0, sizeof(int), h->stream));
-    h->have_state = true; h->smax_valid = false;
+    h->have_state = true; h->smax_valid = false; h->ghosts_valid = false;
     return HYDRO_OK;
 }
 
@@ -962,6 +1001,7 @@ int hydro_substep(hydro_t *h, int stage, double dt, int part)
     }
     if (hi_begin < lo_end) hi_begin = lo_end;
     const bool first = part != 2;                                // the launch that opens the substep
+    if (stage == 1 && first && (rc = ensure_ghosts(h))) return rc;
     if (stage == 1 && first) {
         const int axes = fill_axes(h);
         if (axes) { if ((rc = launch_ghost_fill(h, h->A, true, dev_dt, axes))) return rc; }

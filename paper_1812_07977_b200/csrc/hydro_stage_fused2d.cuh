@@ -11,13 +11,13 @@
 //                wait_O  tile(c+1), x/y fluxes, edge fluxes  arrive_F  wait_F  update
 // No register pipeline (nothing is carried between tiles but the own primitives of the next one),
 // boundary rules in the kernel as in 3D (outflow / reflecting x, y from the source cell; periodic
-// axes from memory ghosts).
+// axes from memory ghosts that the update keeps current).
 #pragma once
 #include "hydro_stage_fused.cuh"
 
 namespace hyd {
 
-template <int STAGE, bool ANISO>
+template <int STAGE, bool ANISO, bool WRAP>
 __global__ void __launch_bounds__(FTX * 16, 1)
 stage_fused2d_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 {
@@ -252,6 +252,25 @@ stage_fused2d_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a
         if (active) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg] = un[v];
+            if (WRAP) {         // periodic x / y: the producer also writes the ghost images of its cell
+                const int i = i0 + tx, j = j0 + ty;
+                if ((a.wrap & 1) && i < NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg + g.nx] = un[v];
+                }
+                if ((a.wrap & 1) && i >= g.nx - NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg - g.nx] = un[v];
+                }
+                if ((a.wrap & 2) && j < NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg + (long long)g.px * g.ny] = un[v];
+                }
+                if ((a.wrap & 2) && j >= g.ny - NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg - (long long)g.px * g.ny] = un[v];
+                }
+            }
             if (STAGE == 2 && a.red) {
 #ifdef HYDRO_VERIFY
                 const double s = cell_signal_speed(un[0], un[1], un[2], un[3], un[4], gamma, gm1, bad);
@@ -291,12 +310,13 @@ inline int fused2d_choose_lz(const Grid &g, int nsm)
 inline cudaError_t plan_stage_fused2d(FusedPlan &p, const Grid &g, const double *A, const double *B, int lz_req = 0)
 {
     cudaError_t e;
-    for (int k = 0; k < 4; ++k) {
-        const void *f = k == 0 ? (const void *)stage_fused2d_kernel<1, false> : k == 1 ? (const void *)stage_fused2d_kernel<1, true>
-                      : k == 2 ? (const void *)stage_fused2d_kernel<2, false> : (const void *)stage_fused2d_kernel<2, true>;
+    const void *fns[8] = { (const void *)stage_fused2d_kernel<1, false, false>, (const void *)stage_fused2d_kernel<1, true, false>,
+                           (const void *)stage_fused2d_kernel<2, false, false>, (const void *)stage_fused2d_kernel<2, true, false>,
+                           (const void *)stage_fused2d_kernel<1, false, true>, (const void *)stage_fused2d_kernel<1, true, true>,
+                           (const void *)stage_fused2d_kernel<2, false, true>, (const void *)stage_fused2d_kernel<2, true, true> };
+    for (const void *f : fns)
         if ((e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FusedSmem<16>::BYTES)) != cudaSuccess)
             return e;
-    }
     int nsm = 148, dev = 0;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
     const int ntile = (g.ny + 15) / 16;
@@ -315,18 +335,24 @@ inline cudaError_t plan_stage_fused2d(FusedPlan &p, const Grid &g, const double 
 template <int STAGE>
 inline cudaError_t launch_stage_fused2d(const FusedPlan &p, const Grid &g, const double *in, const double *old,
                                         double *out, double r, const StepScalars *dev_dt, double dx,
-                                        StepScalars *red, int inbc, cudaStream_t stream)
+                                        StepScalars *red, int inbc, int wrap, cudaStream_t stream)
 {
     if (!p.ready) return cudaErrorNotReady;
     const int b = in == p.base[0] ? 0 : 1;
     if (in != p.base[b]) return cudaErrorInvalidValue;
     FusedArgs a;
     a.g = g; a.Uold = old; a.Uout = out; a.dt_over_dx = r; a.dev_dt = dev_dt; a.dx = dx;
-    a.red = red; a.lz = p.lz; a.inbc = inbc & 3; a.zc0 = 0;
-    if (g.ry != 1.0)
-        stage_fused2d_kernel<STAGE, true><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
-    else
-        stage_fused2d_kernel<STAGE, false><<<p.grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
+    a.red = red; a.lz = p.lz; a.inbc = inbc & 3; a.wrap = wrap; a.zc0 = 0;
+    const dim3 tb(FTX, 16);
+    const size_t smem = FusedSmem<16>::BYTES;
+    const bool aniso = g.ry != 1.0;
+    if (wrap) {
+        if (aniso) stage_fused2d_kernel<STAGE, true, true><<<p.grid, tb, smem, stream>>>(p.map[b], a);
+        else       stage_fused2d_kernel<STAGE, false, true><<<p.grid, tb, smem, stream>>>(p.map[b], a);
+    } else {
+        if (aniso) stage_fused2d_kernel<STAGE, true, false><<<p.grid, tb, smem, stream>>>(p.map[b], a);
+        else       stage_fused2d_kernel<STAGE, false, false><<<p.grid, tb, smem, stream>>>(p.map[b], a);
+    }
     return cudaGetLastError();
 }
 

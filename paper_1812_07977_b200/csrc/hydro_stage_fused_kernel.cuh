@@ -13,6 +13,8 @@ struct FusedArgs {
     StepScalars *red;       // stage 2: max-signal-speed accumulator + sticky flag (or nullptr)
     int lz;                 // planes per z-chunk
     int zc0;                // first z-chunk of this launch (a launch may cover a range of chunks)
+    int wrap;               // bit 0 / 1: x / y is periodic and this kernel maintains its ghost layers: every
+                            // updated cell within two cells of such a face is also stored to its ghost image
     int inbc;               // bit a: the boundary rule of axis a is applied by this kernel (ghost layers of
                             // that axis are never read from memory); 0: all ghosts come from memory
 };
@@ -44,8 +46,10 @@ __device__ __forceinline__ double flip_sign(double x, bool f)
 // (clamp / mirror / wrap); x and y ghost cells of outflow and reflecting faces are read from their
 // source cell inside the tile when the primitives are formed (own-cell source `wsrc` of the threads
 // that stand in for ghost cells, index map of the halo cells), with the normal momentum negated at
-// a wall.  Periodic x / y ghosts need cells from the far side of the domain and are still filled in
-// memory by ghost_fill_kernel (those axes are not in `inbc`).
+// a wall.  Periodic x / y ghosts need cells from the far side of the domain, outside the tile's box:
+// they stay in memory (those axes are not in `inbc`) and are kept current by the PRODUCER -- the
+// update stores every cell within two cells of a periodic face a second time, at its ghost image
+// (`wrap`); ghost_fill_kernel only runs once after the state was set from outside.
 //
 // Synchronisation.  The x/y exchange of one plane needs block-wide hand-offs (primitives, outer
 // face values, fluxes).  Each is a split-phase mbarrier: a warp ARRIVES as soon as its stores are
@@ -59,7 +63,7 @@ __device__ __forceinline__ double flip_sign(double x, bool f)
 //   TY = 8 (two blocks per SM, single primitive tile):
 //     per cell plane c:  wait_W  x/y slopes  arrive_O  [prim(c+4), z-slope]  wait_O  fluxes  arrive_F
 //                        [z-flux, tile(c+1), arrive_W(c+1)]  wait_F  update
-template <int STAGE, int TY, int MINB, bool ANISO>
+template <int STAGE, int TY, int MINB, bool ANISO, bool WRAP>
 __global__ void __launch_bounds__(FTX * TY, MINB)
 stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 {
@@ -366,6 +370,25 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         if (active) {
 #pragma unroll
             for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg] = un[v];
+            if (WRAP) {         // periodic x / y: the producer also writes the ghost images of its cell
+                const int i = i0 + tx, j = j0 + ty;
+                if ((a.wrap & 1) && i < NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg + g.nx] = un[v];
+                }
+                if ((a.wrap & 1) && i >= g.nx - NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg - g.nx] = un[v];
+                }
+                if ((a.wrap & 2) && j < NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg + (long long)g.px * g.ny] = un[v];
+                }
+                if ((a.wrap & 2) && j >= g.ny - NG) {
+#pragma unroll
+                    for (int v = 0; v < 5; ++v) a.Uout[v * sv + cg - (long long)g.px * g.ny] = un[v];
+                }
+            }
             if (STAGE == 2 && a.red) {
 #ifdef HYDRO_VERIFY
                 const double s = cell_signal_speed(un[0], un[1], un[2], un[3], un[4], gamma, gm1, bad);

@@ -16,12 +16,15 @@ struct FusedPlan {
 template <int STAGE, int TY, int MINB>
 inline cudaError_t fused_set_attr()
 {
-    cudaError_t e = cudaFuncSetAttribute(stage_fused_kernel<STAGE, TY, MINB, false>,
-                                         cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)FusedSmem<TY>::BYTES);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(stage_fused_kernel<STAGE, TY, MINB, true>,
-                                cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FusedSmem<TY>::BYTES);
+    const void *fns[4] = { (const void *)stage_fused_kernel<STAGE, TY, MINB, false, false>,
+                           (const void *)stage_fused_kernel<STAGE, TY, MINB, true, false>,
+                           (const void *)stage_fused_kernel<STAGE, TY, MINB, false, true>,
+                           (const void *)stage_fused_kernel<STAGE, TY, MINB, true, true> };
+    for (const void *f : fns) {
+        cudaError_t e = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FusedSmem<TY>::BYTES);
+        if (e != cudaSuccess) return e;
+    }
+    return cudaSuccess;
 }
 
 inline void fused_geometry(FusedPlan &p, const Grid &g, int ty, int lz)
@@ -96,25 +99,29 @@ template <int STAGE>
 inline cudaError_t launch_stage_fused(const FusedPlan &p, const Grid &g, const double *in,
                                       const double *old, double *out, double r,
                                       const StepScalars *dev_dt, double dx, StepScalars *red,
-                                      int inbc, cudaStream_t stream, int zc0 = 0, int nzc = -1)
+                                      int inbc, int wrap, cudaStream_t stream, int zc0 = 0, int nzc = -1)
 {
     if (!p.ready) return cudaErrorNotReady;
     const int b = in == p.base[0] ? 0 : 1;
     if (in != p.base[b]) return cudaErrorInvalidValue;
     FusedArgs a;
     a.g = g; a.Uold = old; a.Uout = out; a.dt_over_dx = r; a.dev_dt = dev_dt; a.dx = dx;
-    a.red = red; a.lz = p.lz; a.inbc = inbc; a.zc0 = zc0;
+    a.red = red; a.lz = p.lz; a.inbc = inbc; a.wrap = wrap; a.zc0 = zc0;
     dim3 grid = p.grid;
     if (nzc >= 0) grid.z = (unsigned)nzc;                     // a range of z-chunks (slab runs: interface chunks first)
     if (grid.z == 0) return cudaSuccess;
     const bool aniso = g.ry != 1.0 || g.rz != 1.0;            // non-cubic cells: two more DMUL per variable
+    // template switches keep the common case (cubic cells, no periodic x / y) free of their code
+#define HYD_LAUNCH(TYv, MINBv, AN, WR)                                                              \
+    stage_fused_kernel<STAGE, TYv, MINBv, AN, WR><<<grid, dim3(FTX, TYv), FusedSmem<TYv>::BYTES, stream>>>(p.map[b], a)
     if (p.ty == 16) {
-        if (aniso) stage_fused_kernel<STAGE, 16, 1, true><<<grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
-        else       stage_fused_kernel<STAGE, 16, 1, false><<<grid, dim3(FTX, 16), FusedSmem<16>::BYTES, stream>>>(p.map[b], a);
+        if (wrap) { if (aniso) HYD_LAUNCH(16, 1, true, true); else HYD_LAUNCH(16, 1, false, true); }
+        else      { if (aniso) HYD_LAUNCH(16, 1, true, false); else HYD_LAUNCH(16, 1, false, false); }
     } else {
-        if (aniso) stage_fused_kernel<STAGE, 8, 2, true><<<grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
-        else       stage_fused_kernel<STAGE, 8, 2, false><<<grid, dim3(FTX, 8), FusedSmem<8>::BYTES, stream>>>(p.map[b], a);
+        if (wrap) { if (aniso) HYD_LAUNCH(8, 2, true, true); else HYD_LAUNCH(8, 2, false, true); }
+        else      { if (aniso) HYD_LAUNCH(8, 2, true, false); else HYD_LAUNCH(8, 2, false, false); }
     }
+#undef HYD_LAUNCH
     return cudaGetLastError();
 }
 
