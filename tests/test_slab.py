@@ -219,3 +219,21 @@ def test_slab_ranks_two_processes_over_gloo_bit_identical(tmp_path):
     out = _torchrun(script, 2, 29623)
     assert out.returncode == 0, (out.stdout[-1500:], out.stderr[-3000:])
     assert "rank0 ok" in out.stdout and "rank1 ok" in out.stdout
+
+
+@pytest.mark.gpu
+def test_bench_slab_mode_two_ranks_share_one_gpu_over_gloo():
+    """bench.py --decomp slab end to end: two slab ranks of one 32 x 32 x 64 domain (they share the
+    GPU and meet only on the host), one JSON line from rank 0."""
+    import json
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", "29624", "bench.py", "--gpus", "2", "--decomp", "slab",
+           "--config", "0", "--steps", "10", "--warmup", "3"]
+    env = dict(os.environ, HYDRO_BENCH_BACKEND="gloo", OMP_NUM_THREADS="2")
+    out = subprocess.run(cmd, cwd=ROOT, env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-3000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["value"] > 0 and d["devices_shared"] and "z-slabs" in d["config"]["parallelism"]
+    assert d["gpu_launches"] >= 10 * 5
