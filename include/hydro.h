@@ -208,12 +208,21 @@ int hydro_ghost_fill(hydro_t *h);
 int hydro_get_padded(hydro_t *h, double *Upad);
 /* Tuning hooks of the fused stage kernel (tests and measurement; defaults are chosen per grid).
  * hydro_set_tiling: tile_rows = 8 | 16 (rows of 32 cells per block; 0 = chosen by the library),
- * planes_per_chunk = z-planes a block marches over (0 = chosen so that the blocks fill whole waves
- * of the SMs; for a 2D run: 32 x 16 tiles a block walks down y).  hydro_get_tiling reports the geometry in use and the number of blocks per stage
- * launch (any out-pointer may be NULL).  hydro_set_graph_replay(h, 0) makes hydro_run_steps /
+ * planes_per_chunk = z-planes a block marches over (for a 2D run: 32 x 16 tiles a block walks down y);
+ * 0 = chosen by the library: uniform chunks that fill whole waves of the SMs, or "balanced layers" --
+ * chunks that put one block on every resident slot of the device plus thinner remainder chunks for
+ * the slots left over ("Launch geometry").  hydro_get_tiling reports the geometry
+ * in use -- planes_per_chunk is the (primary) chunk length -- and the number of blocks per stage launch
+ * (any out-pointer may be NULL).  hydro_tiling_partition is the host logic behind it, callable without a
+ * device: the z partition of a launch over the active planes [kb, ke) of an nx x ny x nz grid on a device
+ * with `sms` multiprocessors, out = { lz, km, nprim, lzr, nlayer }: layers 0 .. nprim-1 are the chunks of
+ * lz planes of [kb, km), layers nprim .. nlayer-1 the chunks of lzr planes of [km, ke).
+ * hydro_set_graph_replay(h, 0) makes hydro_run_steps /
  * hydro_evolve enqueue plain launches instead of replaying the captured one-step CUDA graph. */
 int hydro_set_tiling(hydro_t *h, int tile_rows, int planes_per_chunk);
 int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long long *blocks);
+int hydro_tiling_partition(int nx, int ny, int nz, int tile_rows, int planes_per_chunk, int sms, int kb, int ke,
+                           int out[5]);
 int hydro_set_graph_replay(hydro_t *h, int enable);
 /* Select the stage-kernel implementation (2D and 3D runs; a 1D run always uses 0):
  * 0 = reference-structured simple kernel (one thread per

@@ -20,7 +20,7 @@ SYMBOLS = ["hydro_create", "hydro_create_nd", "hydro_set_state", "hydro_cfl_dt",
            "hydro_get_state", "hydro_destroy", "hydro_set_cfl", "hydro_set_limiter_theta",
            "hydro_get_time", "hydro_max_signal_speed", "hydro_set_stream", "hydro_set_allocator",
            "hydro_run_steps", "hydro_ghost_fill", "hydro_get_padded", "hydro_set_kernel_variant",
-           "hydro_set_tiling", "hydro_get_tiling", "hydro_set_graph_replay",
+           "hydro_set_tiling", "hydro_get_tiling", "hydro_tiling_partition", "hydro_set_graph_replay",
            "hydro_create_slab", "hydro_substep", "hydro_halo_count", "hydro_halo_pack",
            "hydro_halo_unpack", "hydro_halo_push", "hydro_state_base", "hydro_smax_device",
            "hydro_reduce_smax", "hydro_host_alloc", "hydro_update_device", "hydro_update_host",
@@ -80,6 +80,7 @@ def load_library(verify=False):
     L.hydro_set_tiling.argtypes = [vp, C.c_int, C.c_int]
     L.hydro_get_tiling.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.hydro_set_graph_replay.argtypes = [vp, C.c_int]
+    L.hydro_tiling_partition.argtypes = [C.c_int] * 8 + [C.POINTER(C.c_int)]
     L.hydro_create_slab.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int),
                                     C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.hydro_substep.argtypes = [vp, C.c_int, C.c_double, C.c_int]
@@ -101,6 +102,26 @@ def load_library(verify=False):
     L.hydro_last_error.restype = C.c_char_p
     _libs[key] = L
     return L
+
+
+def tiling_partition(nx, ny, nz, tile_rows, planes_per_chunk=0, sms=148, kb=0, ke=None, verify=False):
+    """Host logic of the fused kernel's launch geometry (no device needed): the layers of a launch over the
+    active planes [kb, ke) as a list of (k0, k1), and the raw (lz, km, nprim, lzr, nlayer)."""
+    L = load_library(verify)
+    ke = nz if ke is None else ke
+    out = (C.c_int * 5)()
+    rc = L.hydro_tiling_partition(nx, ny, nz, tile_rows, planes_per_chunk, sms, kb, ke, out)
+    if rc:
+        raise HydroError(rc, "hydro_tiling_partition", L.hydro_last_error().decode())
+    lz, km, nprim, lzr, nlayer = list(out)
+    layers = []
+    for z in range(nlayer):
+        if z < nprim:
+            k0 = kb + z * lz; k1 = min(k0 + lz, km)
+        else:
+            k0 = km + (z - nprim) * lzr; k1 = min(k0 + lzr, ke)
+        layers.append((k0, k1))
+    return layers, (lz, km, nprim, lzr, nlayer)
 
 
 def use_torch_allocator(L, enable=True):

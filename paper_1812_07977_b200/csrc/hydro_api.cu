@@ -225,8 +225,7 @@ int launch_cfl_reduce(hydro *h)
     return HYDRO_OK;
 }
 
-// One substep over the active planes [kb, ke) (whole grid: 0, nz).  The fused kernel works in
-// z-chunks of plan.lz planes, so kb and ke must be chunk boundaries (or nz).
+// One substep over the active planes [kb, ke) (whole grid: 0, nz).
 // After the state was set from outside, the periodic x / y ghost layers of A are filled once.
 int ensure_ghosts(hydro *h)
 {
@@ -266,9 +265,8 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
         if (e2 != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused2d: %s%s", cudaGetErrorString(e2));
         return HYDRO_OK;
     }
-    const int lz = h->plan.lz;
     cudaError_t e = launch_stage_fused<STAGE>(h->plan, g, in, old, out, r, dd, h->dx, red, inbc, wrap_axes(h),
-                                              h->stream, kb / lz, (ke - kb + lz - 1) / lz);
+                                              h->stream, kb, ke);
     g_launches.fetch_add(1, std::memory_order_relaxed);
     if (e != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused: %s%s", cudaGetErrorString(e));
     return HYDRO_OK;
@@ -614,6 +612,19 @@ int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long lon
     if (tile_rows) *tile_rows = h->plan.ty;
     if (planes_per_chunk) *planes_per_chunk = h->plan.lz;
     if (blocks) *blocks = (long long)h->plan.grid.x * h->plan.grid.y * h->plan.grid.z;
+    return HYDRO_OK;
+}
+
+int hydro_tiling_partition(int nx, int ny, int nz, int tile_rows, int planes_per_chunk, int sms, int kb, int ke,
+                           int out[5])
+{
+    if (nx < 1 || ny < 1 || nz < 1 || (tile_rows != 8 && tile_rows != 16) || planes_per_chunk < 0 || sms < 1 ||
+        kb < 0 || ke > nz || ke <= kb || !out)
+        return fail(HYDRO_ERR_ARG, "tiling_partition: bad argument%s%s");
+    Grid g{};
+    g.nx = nx; g.ny = ny; g.nz = nz;
+    const FusedLayers z = fused_partition(g, tile_rows, kb, ke, sms, planes_per_chunk);
+    out[0] = z.lz; out[1] = z.km; out[2] = z.nprim; out[3] = z.lzr; out[4] = z.nlayer;
     return HYDRO_OK;
 }
 
@@ -992,7 +1003,7 @@ int hydro_substep(hydro_t *h, int stage, double dt, int part)
     const double r = dt / h->dx;
     // interface planes: the z-chunks (fused kernel) or plane pairs (simple kernel) next to a
     // neighbouring slab; computed first so that their exchange overlaps the interior
-    const int unit = (h->variant == 0 || g.ndim < 3) ? 2 : h->plan.lz;
+    const int unit = (h->variant == 0 || g.ndim < 3) ? 2 : (h->plan.km < g.nz ? FUSED_SLAB_UNIT : h->plan.lz);
     int lo_end = 0, hi_begin = g.nz;
     if (g.bc[4] == HYDRO_BC_NEIGHBOUR) lo_end = unit < g.nz ? unit : g.nz;
     if (g.bc[5] == HYDRO_BC_NEIGHBOUR) {

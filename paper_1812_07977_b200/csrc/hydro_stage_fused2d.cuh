@@ -342,7 +342,7 @@ inline cudaError_t launch_stage_fused2d(const FusedPlan &p, const Grid &g, const
     if (in != p.base[b]) return cudaErrorInvalidValue;
     FusedArgs a;
     a.g = g; a.Uold = old; a.Uout = out; a.dt_over_dx = r; a.dev_dt = dev_dt; a.dx = dx;
-    a.red = red; a.lz = p.lz; a.inbc = inbc & 3; a.wrap = wrap; a.zc0 = 0;
+    a.red = red; a.lz = p.lz; a.inbc = inbc & 3; a.wrap = wrap; a.zc0 = 0; a.kb = 0; a.km = 0; a.ke = 0; a.nprim = 0; a.lzr = 1;
     const dim3 tb(FTX, 16);
     const size_t smem = FusedSmem<16>::BYTES;
     const bool aniso = g.ry != 1.0;

@@ -3,6 +3,12 @@
 
 namespace hyd {
 
+// Layers.  blockIdx.x / .y = tile, blockIdx.z = layer: the planes [kb, km) in chunks of lz planes and,
+// when km < ke, the planes [km, ke) in thinner chunks of lzr planes.  Uniform chunking has km = ke; the
+// balanced partition (hydro_stage_fused_plan.cuh) makes the chunks of [kb, km) fill the resident slots
+// of the device once and hands the remainder to the slots left over.  Neighbouring tiles of a layer
+// sweep z in lockstep and share their halo columns in L2.
+
 struct FusedArgs {
     Grid g;
     const double *Uold;     // stage 2: U0 (read at the thread's own cell only); may alias Uout
@@ -11,8 +17,10 @@ struct FusedArgs {
     const StepScalars *dev_dt;
     double dx;
     StepScalars *red;       // stage 2: max-signal-speed accumulator + sticky flag (or nullptr)
-    int lz;                 // planes per z-chunk
-    int zc0;                // first z-chunk of this launch (a launch may cover a range of chunks)
+    int lz;                 // planes per z-chunk (2D: tile rows per chunk)
+    int zc0;                // 2D kernel only
+    int kb, km, ke;         // 3D: this launch updates the active planes [kb, ke): layers blockIdx.z < nprim are the
+    int nprim, lzr;         // chunks of lz planes of [kb, km), the others the chunks of lzr planes of [km, ke)
     int wrap;               // bit 0 / 1: x / y is periodic and this kernel maintains its ghost layers: every
                             // updated cell within two cells of such a face is also stored to its ghost image
     int inbc;               // bit a: the boundary rule of axis a is applied by this kernel (ghost layers of
@@ -80,8 +88,9 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
     const Grid &g = a.g;
     const int tx = threadIdx.x, ty = threadIdx.y, t = ty * TX + tx;
     const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;     // tile origin, active coordinates
-    const int k0 = (blockIdx.z + a.zc0) * a.lz;
-    const int k1 = min(k0 + a.lz, g.nz);                      // chunk = active planes [k0, k1)
+    const int zl = blockIdx.z, zr = zl - a.nprim;             // chunk = active planes [k0, k1)
+    const int k0 = zr < 0 ? a.kb + zl * a.lz : a.km + zr * a.lzr;
+    const int k1 = zr < 0 ? min(k0 + a.lz, a.km) : min(k0 + a.lzr, a.ke);
     const int nc = k1 - k0;                                   // cell planes; raw planes 0..nc+3
     const int nplanes = nc + 4;                               //   (raw plane p = active plane k0-2+p)
     const double gamma = g.gamma, gm1 = g.gm1, igm1 = g.igm1, theta = g.theta;
@@ -283,7 +292,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
             HYD_PRIM5(Un, gm1, Wn);
             HYD_LIMITED_FACES(theta, Wa, Wb, Wn, Iz, Ozn);
         }
-        tma::mbar_wait(barO, par);
+        tma::mbar_wait_sync(barO, par);
         if (PIPE) __syncwarp();                               // the warp's own outer x values are in place
         // every warp is past P4 of cell plane c-1: raw plane c+1 is dead, refill its stage
         if (t == 0 && c + 5 < nplanes) { tma::fence_proxy_async(); request_plane(c + 5); }
@@ -356,7 +365,7 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
 #pragma unroll
             for (int v = 0; v < 5; ++v) u1r[v] = Uk[v * S::WSZ + wc];
         }
-        tma::mbar_wait(barF, par);
+        tma::mbar_wait_sync(barF, par);
         // ---- P4: divergence, RK combine, store, CFL ------------------------------------------
         double un[5];
 #pragma unroll

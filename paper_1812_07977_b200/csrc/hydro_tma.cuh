@@ -59,6 +59,27 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         : "memory");
 }
 
+// Wait on a block-wide hand-off barrier: try_wait with a suspend-time hint, so that a warp that finds the
+// phase incomplete is parked by the hardware for up to ~200 ns instead of re-polling at once (measured:
+// the flux barrier is polled 29 times per warp and plane without the hint; with it 256^3 runs 1.5 % and
+// 128^3 2 % faster).  The TMA waits keep the plain form: the data has almost always landed.
+#ifndef HYD_WAIT_HINT
+#define HYD_WAIT_HINT 200
+#endif
+__device__ __forceinline__ void mbar_wait_sync(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred P1;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, %2;\n"
+        "@P1 bra DONE;\n"
+        "bra LAB_WAIT;\n"
+        "DONE:\n"
+        "}" ::"r"(smem_u32(bar)), "r"(parity), "r"((uint32_t)HYD_WAIT_HINT)
+        : "memory");
+}
+
 // one rank-4 box: coordinates (c0 fastest) -> shared memory at dst, completion on bar
 __device__ __forceinline__ void load_4d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, int c3,
                                         uint64_t *bar)

@@ -67,3 +67,46 @@ def test_product_package_never_imports_the_oracle():
                 text = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in text and "from oracle" not in text, f
                 assert "liboracle" not in text, f
+
+
+def test_tiling_partition_covers_every_plane_once(libs):
+    """Host logic of the fused kernel's launch geometry (hydro_tiling_partition, no device): whatever the
+    grid, the tile height, the requested chunk length and the plane range, the layers tile [kb, ke)
+    exactly, in order, without empty layers -- the same arithmetic the kernel uses to find its chunk."""
+    import random
+    rnd = random.Random(7)
+    cases = [(256, 256, 256, 16, 0, 148, 0, 256), (128, 128, 128, 16, 0, 148, 0, 128), (32, 32, 32, 8, 0, 148, 0, 32),
+             (512, 512, 512, 16, 0, 148, 0, 512), (160, 160, 160, 16, 0, 148, 0, 160), (33, 257, 65, 16, 0, 148, 0, 65),
+             (64, 64, 2048, 16, 0, 148, 16, 2032), (2, 2, 2, 8, 0, 148, 0, 2), (100, 70, 45, 8, 7, 148, 0, 45)]
+    for _ in range(300):
+        nx, ny, nz = (rnd.randint(2, 600), rnd.randint(2, 600), rnd.randint(2, 700))
+        kb = rnd.choice([0, 0, rnd.randint(0, nz - 1)])
+        ke = rnd.choice([nz, nz, rnd.randint(kb + 1, nz)])
+        cases.append((nx, ny, nz, rnd.choice([8, 16]), rnd.choice([0, 0, 0, rnd.randint(1, nz)]),
+                      rnd.choice([148, 148, 132, 1, 7]), kb, ke))
+    for nx, ny, nz, ty, lzreq, sms, kb, ke in cases:
+        layers, (lz, km, nprim, lzr, nlayer) = binding.tiling_partition(nx, ny, nz, ty, lzreq, sms, kb, ke)
+        assert len(layers) == nlayer >= 1 and lz >= 1 and lzr >= 1 and kb < km <= ke, (nx, ny, nz, ty, lzreq, sms)
+        assert layers[0][0] == kb and layers[-1][1] == ke
+        for (a0, a1), (b0, b1) in zip(layers, layers[1:]):
+            assert a1 == b0
+        assert all(k1 > k0 for k0, k1 in layers), (layers, nx, ny, nz, ty, lzreq, sms, kb, ke)
+        if lzreq:
+            assert km == ke and lz == min(lzreq, ke - kb)
+
+
+def test_tiling_partition_balances_the_paper_sizes(libs):
+    """256^3 per GPU is the paper's benchmark size and 128^3 its production size: on 148
+    SMs with 32 x 16 tiles the balanced layers put one thick chunk of every tile on its own SM and hand
+    the thin remainder to the SMs left over, instead of 6.9 / 0.86 waves of uniform 32-plane chunks."""
+    for n, tiles in ((256, 128), (128, 32)):
+        layers, (lz, km, nprim, lzr, nlayer) = binding.tiling_partition(n, n, n, 16)
+        q = 148 // tiles
+        assert nprim == q and km < n and tiles * nprim <= 148
+        left = 148 - tiles * nprim
+        rest = nlayer - nprim
+        rounds = -(-tiles * rest // left)
+        primary = lz + 1.25
+        remainder = rounds * (lzr + 1.25)
+        assert abs(primary - remainder) <= 0.15 * primary          # the two sides finish together
+        assert primary < 1.06 * (n * tiles / 148 + 1.25)            # within 6 % of a perfect split
