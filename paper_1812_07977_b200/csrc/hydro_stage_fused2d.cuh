@@ -183,7 +183,7 @@ stage_fused2d_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a
             load_own(sm + S::OFF_RING + (p % FNS) * S::STAGE, (t0 + p) * TY, Un);
             HYD_PRIM5(Un, gm1, Wn);
         }
-        tma::mbar_wait(barO, par);
+        tma::mbar_wait_sync(barO, par);
         __syncwarp();
         // every warp is past the update of tile c-1: its raw tile is dead, refill that stage
         if (t == 0 && c >= 1 && c + 3 < nc) { tma::fence_proxy_async(); request_tile(c + 3); }
@@ -231,7 +231,7 @@ stage_fused2d_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a
 #pragma unroll
             for (int v = 0; v < 5; ++v) Uo[v] = active ? a.Uold[v * sv + cg] : 0.0;
         }
-        tma::mbar_wait(barF, par);
+        tma::mbar_wait_sync(barF, par);
         // ---- divergence (O5, two dimensions: D = dFx + (dx/dy) dFy), RK combine, store, CFL --------
         double un[5];
 #pragma unroll
