@@ -316,6 +316,40 @@ def test_fuzz_small_grids_bitwise():
         g.close()
 
 
+def test_balanced_layers_bitwise():
+    """Launch geometry of DESIGN.md section 6.1 ("balanced layers"): on grids whose partition has thick
+    primary chunks plus thinner remainder chunks (checked through hydro_tiling_partition), and for a
+    sub-range of planes as the slab driver launches it, the verification build still equals the oracle
+    bit for bit and the production build meets the one-step bar -- the partition changes which block
+    computes a plane, never the arithmetic."""
+    import torch
+    from paper_1812_07977_b200 import binding
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    cases = [((70, 200, 40), 16, [OUT, REF, PER, PER, REF, OUT]), ((70, 100, 37), 8, [PER, PER, OUT, OUT, PER, PER]),
+             ((40, 250, 21), 16, [REF, REF, OUT, REF, OUT, OUT])]
+    for k, (shape, ty, bc) in enumerate(cases):
+        layers, (lz, km, nprim, lzr, nlayer) = binding.tiling_partition(*shape, ty, 0, sms)
+        if sms == 148:
+            assert km < shape[2] and nlayer > nprim, (shape, ty, layers)     # a remainder layer is in play
+        U = inputs.random_state(*shape, gamma=1.4, seed=300 + k, vamp=0.4)
+        c = _cpu(shape, 1.4, 1.0 / shape[0], bc, 0.6, 1.4)
+        c.set_state(U)
+        for _ in range(2):
+            c.step(c.cfl_dt())
+        want = c.get_state()
+        g = _gpu(shape, 1.4, 1.0 / shape[0], bc, 0.6, 1.4, verify=True)
+        g.set_tiling(ty, 0)
+        assert g.get_tiling()["blocks"] == nlayer * -(-shape[0] // 32) * -(-shape[1] // ty)
+        g.set_state(U); g.run_steps(2)
+        assert np.array_equal(g.get_state(), want), (shape, ty)
+        g.close()
+        g = _gpu(shape, 1.4, 1.0 / shape[0], bc, 0.6, 1.4, verify=False)
+        g.set_tiling(ty, 0)
+        g.set_state(U); g.run_steps(2)
+        assert_one_step_bar(g.get_state(), want, tol=4e-14)
+        g.close()
+
+
 def test_config1_sod_evolve_to_t02():
     cfg = inputs.config(1)
     U = cfg.state()
