@@ -350,6 +350,34 @@ def test_balanced_layers_bitwise():
         g.close()
 
 
+def test_production_build_long_runs_on_ragged_mixed_boundary_grids():
+    """The production build against the oracle at the END of longer runs on grids that are ragged against
+    every tile and chunk size and mix all three boundary kinds (the full-size configs are cubic with one
+    boundary kind each): 60 device-dt steps of a smooth-plus-noise state, north_star's end-of-run bar,
+    the same number of steps taken, and the verification build still bit-identical after 60 steps."""
+    cases = [((100, 70, 45), [OUT, REF, PER, PER, REF, OUT], 1.4, 0.6),
+             ((33, 257, 65), [REF, REF, OUT, OUT, PER, PER], 5.0 / 3.0, 0.5),
+             ((77, 50, 131), [PER, PER, REF, OUT, OUT, REF], 1.4, 0.7)]
+    for k, (shape, bc, gamma, cfl) in enumerate(cases):
+        U = inputs.random_state(*shape, gamma=gamma, seed=400 + k, vamp=0.3)
+        c = _cpu(shape, gamma, 1.0 / shape[0], bc, cfl, 1.4)
+        c.set_state(U)
+        for _ in range(60):
+            c.step(c.cfl_dt())
+        want = c.get_state()
+        for verify in (False, True):
+            g = _gpu(shape, gamma, 1.0 / shape[0], bc, cfl, 1.4, verify=verify)
+            g.set_state(U); g.run_steps(60)
+            got = g.get_state()
+            if verify:
+                assert np.array_equal(got, want), (shape, bc)
+                assert g.get_time() == c.get_time()
+            else:
+                assert_production_bar(got, want)
+                assert abs(g.get_time()[0] - c.get_time()[0]) <= 1e-12 * c.get_time()[0]
+            g.close()
+
+
 def test_config1_sod_evolve_to_t02():
     cfg = inputs.config(1)
     U = cfg.state()
