@@ -32,9 +32,13 @@ UNIT = "cell-updates/s"
 # algorithmic HBM bytes per cell: stage 1 reads U0 and writes U1 (2 x 40 B),
 # stage 2 reads U1 and U0 and writes U(n+1) (3 x 40 B)
 BYTES_STAGE = {1: 80.0, 2: 120.0}
-# algorithmic fp64-pipe instructions per cell per stage and the measured
-# fp64 pipe peak: 63 lanes/clk/SM x 148 SM at clocks.max.sm (DFMA/DADD/DMUL microbenchmark)
-FP64_INSTR_STAGE = {1: 406.0, 2: 446.0}
+# algorithmic fp64-pipe instructions per cell per stage (primitives 13, 15 slopes
+# x 9, 3 HLL fluxes x 62, update 30 / 40, fused signal speed 0 / 31; each slope and face once, no halo)
+# and the measured fp64 pipe peak: 63 lanes/clk/SM x 148 SM at clocks.max.sm (DFMA/DADD/DMUL microbenchmark)
+FP64_INSTR_STAGE = {1: 364.0, 2: 405.0}
+# shared-memory crossbar: 128 B/clk/SM; bytes the threads and the TMA unit move through it per cell and
+# stage (86 eight-byte accesses per thread and plane + the 36 x 20 x 40 B box)
+SMEM_BYTES_CELL_STAGE = 86 * 8.0 + 36 * 20 * 40.0 / 512
 FP64_LANES_PER_SM, N_SM = 63, 148
 
 
@@ -327,7 +331,7 @@ def run_ours(args):
     _, nsteps = h.get_time()
     st_ms = kt["stage1"][0] + kt["stage2"][0]
     st_n = kt["stage1"][1] + kt["stage2"][1]
-    roofline = roofline_hbm = None
+    roofline = roofline_alu = None
     if st_n:
         bytes_pair = (BYTES_STAGE[1] + BYTES_STAGE[2]) * cells     # one stage-1 + one stage-2 launch
         avg_pair_ms = st_ms / (st_n / 2)
@@ -339,27 +343,32 @@ def run_ours(args):
                   "timed_in": "second pass of the same K steps with per-kernel CUDA events on the "
                               "library's stream (direct launches), %.4f ms per step" % (ms_prof / args.steps)}
         # HBM view (BASELINE.json's metric): algorithmic bytes of the two stage launches / their time
-        roofline_hbm = dict({"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
-                             "frac": achieved / hbm_peak, "traffic": traffic["dram"],
-                             "traffic_source": traffic["source"], "peak_source": peak_src,
-                             "target": "north_star asks for >= 0.70 of peak HBM in the stage kernels",
-                             "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
-                                                              "stage2": BYTES_STAGE[2] * cells}}, **common)
-        # fp64-pipe view of the same two launches: the roofline that BINDS this kernel (DESIGN.md
-        # section 6.1: 4.3 fp64 instructions per byte against a machine balance of 2.8)
+        # fp64-pipe view of the same two launches
         peak = N_SM * FP64_LANES_PER_SM * sm_max * 1e6 / 1e12
         ach = (FP64_INSTR_STAGE[1] + FP64_INSTR_STAGE[2]) * cells / (avg_pair_ms * 1e-3) / 1e12
-        roofline = dict({"bound": "alu", "achieved": ach, "peak": peak, "unit": "T fp64 thread-instr/s",
-                         "frac": ach / peak, "traffic": traffic["fp64"],
-                         "traffic_source": traffic["source"],
-                         "note": "the kernel saturates neither roofline (latency / issue-slot "
-                                 "limited); both views are reported with equal standing: "
-                                 "roofline (fp64 pipe) and roofline_hbm (BASELINE.json's metric)",
-                         "hbm_frac": achieved / hbm_peak,
-                         "algorithmic_instr_per_cell": FP64_INSTR_STAGE,
-                         "peak_source": "63 fp64 lanes/clk/SM (measured DFMA/DADD/DMUL rate, "
-                                        "profiles/r1_fp64_pipe_microbench.md) x 148 SM x clocks.max.sm"},
+        smem_peak = N_SM * 128.0 * sm_max * 1e6 / 1e9
+        smem_ach = 2 * SMEM_BYTES_CELL_STAGE * cells / (avg_pair_ms * 1e-3) / 1e9
+        # HBM view (BASELINE.json's metric and north_star's target): algorithmic bytes of the two stage
+        # launches / their time.  The kernel saturates no single unit (ablations):
+        # HBM, the shared-memory crossbar and the fp64 pipe are each 40-60 % busy and overlap only partly
+        # at 4 warps per sub-partition; the fractions of the other two are carried along.
+        roofline = dict({"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": achieved / hbm_peak, "traffic": traffic["dram"],
+                         "traffic_source": traffic["source"], "peak_source": peak_src,
+                         "target": "north_star asks for >= 0.70 of peak HBM in the stage kernels",
+                         "algorithmic_bytes_per_launch": {"stage1": BYTES_STAGE[1] * cells,
+                                                          "stage2": BYTES_STAGE[2] * cells},
+                         "fp64_pipe_frac": ach / peak, "smem_crossbar_frac": smem_ach / smem_peak,
+                         "note": "no single unit is saturated: HBM, shared-memory crossbar and fp64 pipe "
+                                 "overlap only partly (DESIGN.md section 6.1); roofline_alu is the fp64 view"},
                         **common)
+        roofline_alu = dict({"bound": "alu", "achieved": ach, "peak": peak, "unit": "T fp64 thread-instr/s",
+                             "frac": ach / peak, "traffic": traffic["fp64"],
+                             "traffic_source": traffic["source"],
+                             "algorithmic_instr_per_cell": FP64_INSTR_STAGE,
+                             "peak_source": "63 fp64 lanes/clk/SM (measured DFMA/DADD/DMUL rate, "
+                                            "profiles/r2_fp64_pipe_microbench.md) x 148 SM x clocks.max.sm"},
+                            **common)
 
     # ---- the named ABI loop, state resident: K x (hydro_cfl_dt + hydro_step(dt)), i.e. one 32-byte
     #      device->host read and a stream sync per step (SURVEY.md section 8(d) variant (i)) ----------
@@ -445,7 +454,7 @@ def run_ours(args):
                 "abi_loop": {"value": world * cells * args.steps / (ms_abi * 1e-3), "unit": UNIT,
                              "ms_per_step": ms_abi / args.steps,
                              "what": "K x (hydro_cfl_dt + hydro_step(dt)), state resident in HBM"},
-                "roofline": roofline, "roofline_hbm": roofline_hbm, "cpu_baseline": cpu}
+                "roofline": roofline, "roofline_alu": roofline_alu, "cpu_baseline": cpu}
         n_dev = torch.cuda.device_count()
         if backend != "nccl" or world > n_dev:
             # replicas share devices (HYDRO_BENCH_BACKEND=gloo plumbing test): not a multi-GPU figure

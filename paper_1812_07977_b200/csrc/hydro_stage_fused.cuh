@@ -6,7 +6,8 @@
 // ComputeFluxes / ComputeUpdate and the "FluidCurrent = ..." lines of Algorithm 1
 // without any of its intermediate storages.
 //
-// Shape.  The kernel is bound by the fp64 pipe, not by HBM, so the design
+// Shape.  The kernel is not bound by HBM (each value crosses it once per stage) but by
+// how well fp64 work, shared-memory exchange and the TMA stream overlap at 16 warps per SM, so the design
 // minimises fp64 instructions per cell: every slope and every face flux is computed exactly once.
 //   * A block owns a TX x TY column tile (x fastest, one warp per x-row of 32 cells) and marches
 //     along z over a chunk of `lz` planes.  A thread owns the column (i, j).
