@@ -224,12 +224,14 @@ int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long lon
 int hydro_tiling_partition(int nx, int ny, int nz, int tile_rows, int planes_per_chunk, int sms, int kb, int ke,
                            int out[5]);
 int hydro_set_graph_replay(hydro_t *h, int enable);
-/* Select the stage-kernel implementation (2D and 3D runs; a 1D run always uses 0):
+/* Select the stage-kernel implementation:
  * 0 = reference-structured simple kernel (one thread per
  * cell, everything recomputed, ghost layers filled in memory before each substep); 1 = fused tiled
- * kernel with the boundary rules applied in the kernel (default: ghost layers are written to memory
- * only for periodic x / y faces, and not at all otherwise -- three launches per step); 2 = the same
- * fused kernel reading every ghost layer from memory (cross-check of 1). */
+ * kernel (default).  2D and 3D runs: the boundary rules are applied in the kernel (ghost layers are
+ * written to memory only for periodic x / y faces, and not at all otherwise -- three launches per
+ * step); 1D runs: each slope and flux once per cell, ghost cells still filled in memory before each
+ * substep.  2 = the fused 2D / 3D kernel reading every ghost layer from memory (cross-check of 1; not
+ * for 1D runs, whose variant 1 already does). */
 int hydro_set_kernel_variant(hydro_t *h, int variant);
 /* Measurement hooks (bench.py): when enabled, every kernel launch of this handle is bracketed by
  * CUDA events on the handle's stream.  hydro_get_kernel_time synchronises and returns the summed

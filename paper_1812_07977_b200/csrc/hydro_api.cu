@@ -6,6 +6,7 @@
 #include "hydro_kernels.cuh"
 #include "hydro_stage_fused.cuh"
 #include "hydro_stage_fused2d.cuh"
+#include "hydro_stage_fused1d.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -168,12 +169,12 @@ int periodic_xy(const hydro *h)
     return axes;
 }
 
-bool fused_run(const hydro *h) { return h->g.ndim >= 2 && h->variant == 1; }
+bool fused_run(const hydro *h) { return h->variant == 1; }
 
 int wrap_axes(const hydro *h)      // periodic axes whose ghost layers the stage kernels maintain
 {
     const long long cells = (long long)h->g.nx * h->g.ny * h->g.nz;
-    return fused_run(h) && cells <= (1ll << 25) ? periodic_xy(h) : 0;
+    return fused_run(h) && h->g.ndim >= 2 && cells <= (1ll << 25) ? periodic_xy(h) : 0;    // (1D: periodic x keeps its fill)
 }
 
 int fill_axes(const hydro *h)      // axes ghost_fill_kernel fills before every stage
@@ -247,7 +248,7 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
     const StepScalars *dd = dev_dt ? h->scal : nullptr;
     StepScalars *red = reduce ? h->scal : nullptr;
     Scope sc(h, STAGE == 1 ? K_STAGE1 : K_STAGE2);
-    if (h->variant == 0 || g.ndim == 1) {     // (variants 1 and 2 are the fused kernels of 2D / 3D runs)
+    if (h->variant == 0) {                    // (variants 1 and 2 are the fused kernels)
         dim3 tb(32, 4, 1);
         if (g.ndim == 1) tb = dim3(128, 1, 1);
         dim3 gr((g.nx + tb.x - 1) / tb.x, (g.ny + tb.y - 1) / tb.y, ke - kb);
@@ -255,6 +256,12 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
         else if (g.ndim == 2) stage_simple_kernel<STAGE, 2><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red, kb);
         else                  stage_simple_kernel<STAGE, 3><<<gr, tb, 0, h->stream>>>(g, in, old, out, r, dd, h->dx, red, kb);
         LAUNCH_CHECK("stage_simple");
+        return HYDRO_OK;
+    }
+    if (g.ndim == 1) {                        // fused 1D kernel
+        cudaError_t e1 = launch_stage_fused1d<STAGE>(g, in, old, out, r, dd, h->dx, red, inkernel_axes(h) & 1, h->stream);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (e1 != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused1d: %s%s", cudaGetErrorString(e1));
         return HYDRO_OK;
     }
     const int inbc = inkernel_axes(h);
@@ -486,7 +493,6 @@ int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, c
         if (a < ndim && d[a] < h->dmin) h->dmin = d[a];
     }
     g.ry = h->dx / h->dxyz[1]; g.rz = h->dx / h->dxyz[2];
-    if (ndim == 1) h->variant = 0;
     // +16 tail so vectorised / TMA reads that run a few doubles past the last row stay inside
     h->buf_doubles = (size_t)LEAD + (size_t)NVAR * g.sv + 16 + 2;
     h->buf_doubles = ((h->buf_doubles + 15) / 16) * 16;
@@ -574,8 +580,8 @@ int hydro_set_limiter_theta(hydro_t *h, double theta)
 int hydro_set_kernel_variant(hydro_t *h, int variant)
 {
     if (!h || variant < 0 || variant > 2) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0, 1 or 2%s%s");
-    if (h->g.ndim == 1 && variant != 0)
-        return fail(HYDRO_ERR_ARG, "set_kernel_variant: 1D runs use the simple kernel (variant 0)%s%s");
+    if (h->g.ndim == 1 && variant == 2)
+        return fail(HYDRO_ERR_ARG, "set_kernel_variant: a 1D run has variants 0 and 1 (its ghost cells always come from memory)%s%s");
     h->variant = variant;
     h->ghosts_valid = false;
     drop_graph(h);

@@ -4,9 +4,10 @@
 
 namespace hyd {
 
-#ifndef FUSED_WARM
-#define FUSED_WARM 1.25
-#endif
+// Cost of a block's start (barrier set-up, first TMA round trip, the four warm-up planes that only cost
+// primitives and z-slopes) in plane times: fit to measured whole-column, 64- and 32-plane chunks at
+// 32 x 16 (2.98 us per plane and stage, 3.7 us per block).
+constexpr double FUSED_WARM = 1.25;
 constexpr int FUSED_SLAB_UNIT = 16;   // balanced layers: planes next to a slab interface that are computed first
 
 // z partition of one launch over the active planes [kb, ke): chunks of lz planes over [kb, km) and,
@@ -51,13 +52,12 @@ inline long long fused_tiles(const Grid &g, int ty)
     return (long long)((g.nx + FTX - 1) / FTX) * ((g.ny + ty - 1) / ty);
 }
 
-// Launch geometry.  A block streams (l + 4) planes for l computed ones, but the four warm-up planes
-// only cost primitives and z-slopes, so with the block prologue a chunk of l planes takes about
-// (l + 2) plane times; blocks are handed to the SMs in waves of (SMs x resident blocks).  Measured on
-// B200 (tiling sweep): the best geometry is the one that fills whole waves,
-// short chunks are cheap, 32 x 16 tiles (one block per SM) beat 32 x 8 tiles (two per SM) at equal
-// wave count because they carry half the halo work, and a lone 32 x 8 block on an SM runs about 1.5
-// times faster than when it shares the SM (tiny grids: more, smaller blocks win).
+// Uniform chunks.  A chunk of l planes takes about (l + FUSED_WARM) plane times; blocks are handed to the
+// SMs in waves of (SMs x resident blocks).  Measured on B200 (tiling sweep): the
+// best uniform chunking is the one that fills whole waves, short chunks are cheap, 32 x 16 tiles (one
+// block per SM) beat 32 x 8 tiles (two per SM) at equal wave count because they carry half the halo work,
+// and a lone 32 x 8 block on an SM runs about 1.5 times faster than when it shares the SM (tiny grids:
+// more, smaller blocks win).
 inline double fused_cost(const Grid &g, int ty, int nzr, int l, int nsm)
 {
     const long long blocks = fused_tiles(g, ty) * ((nzr + l - 1) / l);

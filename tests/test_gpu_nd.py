@@ -31,6 +31,8 @@ def _pair(shape, ndim, dxyz, bc, gamma=1.4, cfl=0.7, theta=None, verify=True, va
 CASES = [
     (1, (257, 1, 1), (0.01, 1.0, 1.0), (OUT, OUT, OUT, OUT, OUT, OUT)),
     (1, (64, 1, 1), (0.3, 1.0, 1.0), (REF, OUT, OUT, OUT, OUT, OUT)),
+    (1, (200001, 1, 1), (1e-5, 1.0, 1.0), (OUT, REF, OUT, OUT, OUT, OUT)),    # fused 1D kernel: more tiles than resident blocks
+    (1, (1000, 1, 1), (1e-3, 1.0, 1.0), (PER, PER, OUT, OUT, OUT, OUT)),       # periodic x keeps its ghost fill
     (1, (2, 1, 1), (0.3, 1.0, 1.0), (PER, PER, OUT, OUT, OUT, OUT)),
     (2, (70, 37, 1), (0.02, 0.02, 1.0), (OUT, REF, PER, PER, OUT, OUT)),
     (2, (33, 5, 1), (0.1, 0.031, 1.0), (PER, PER, REF, OUT, OUT, OUT)),
@@ -46,7 +48,7 @@ CASES = [
 @pytest.mark.parametrize("ndim,shape,dxyz,bc", CASES)
 def test_nd_runs_bit_identical_on_verification_build(ndim, shape, dxyz, bc):
     U = inputs.random_state(*shape, seed=sum(shape) + ndim, vamp=0.5)
-    variants = (1, 2, 0) if ndim >= 2 else (None,)
+    variants = (1, 2, 0) if ndim >= 2 else (1, 0)
     for variant in variants:
         g, c = _pair(shape, ndim, dxyz, bc, variant=variant)
         if ndim == 2 and variant == 2:
@@ -141,7 +143,26 @@ def test_create_nd_status_codes():
     with pytest.raises(HydroError):
         g.set_tiling(8, 4)                                 # 2D runs use 32 x 16 tiles
     g = Hydro(8, 1, 1, 1.4, 0.1, (0,) * 6, ndim=1, dxyz=(0.1, 0.2, 0.1))
+    g.set_kernel_variant(0); g.set_kernel_variant(1)       # 1D runs: simple or fused 1D kernel
     with pytest.raises(HydroError):
-        g.set_kernel_variant(1)                            # 1D runs: simple kernel only
+        g.set_kernel_variant(2)                            # (their ghost cells always come from memory)
     with pytest.raises(HydroError):
         g.set_tiling(16, 4)
+
+
+@pytest.mark.gpu
+def test_1d_launches_per_step():
+    """The fused 1D kernel applies outflow and reflecting ends itself (three launches per step: start of
+    step, two stages); a periodic x keeps its ghost fill (four); the simple kernel always fills (four)."""
+    from paper_1812_07977_b200.binding import Hydro
+    for bc0, variant, want in ((OUT, 1, 3), (REF, 1, 3), (PER, 1, 4), (OUT, 0, 4)):
+        bc = (bc0, bc0, OUT, OUT, OUT, OUT)
+        g = Hydro(500, 1, 1, 1.4, 1.0 / 500, bc, ndim=1)
+        g.set_kernel_variant(variant)
+        g.set_graph_replay(False)
+        g.set_state(inputs.random_state(500, 1, 1, seed=5, vamp=0.3))
+        g.run_steps(1)
+        n0 = g.launch_count()
+        g.run_steps(5)
+        assert g.launch_count() - n0 == 5 * want, (bc0, variant, g.launch_count() - n0)
+        g.close()
