@@ -229,9 +229,9 @@ int hydro_set_graph_replay(hydro_t *h, int enable);
  * cell, everything recomputed, ghost layers filled in memory before each substep); 1 = fused tiled
  * kernel (default).  2D and 3D runs: the boundary rules are applied in the kernel (ghost layers are
  * written to memory only for periodic x / y faces, and not at all otherwise -- three launches per
- * step); 1D runs: each slope and flux once per cell, ghost cells still filled in memory before each
- * substep.  2 = the fused 2D / 3D kernel reading every ghost layer from memory (cross-check of 1; not
- * for 1D runs, whose variant 1 already does). */
+ * step); 1D runs: each slope and flux once per cell, every boundary kind applied in the kernel.
+ * 2 = the fused 2D / 3D kernel reading every ghost layer from memory (cross-check of 1; not for 1D
+ * runs). */
 int hydro_set_kernel_variant(hydro_t *h, int variant);
 /* Measurement hooks (bench.py): when enabled, every kernel launch of this handle is bracketed by
  * CUDA events on the handle's stream.  hydro_get_kernel_time synchronises and returns the summed

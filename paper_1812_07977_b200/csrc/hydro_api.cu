@@ -174,17 +174,19 @@ bool fused_run(const hydro *h) { return h->variant == 1; }
 int wrap_axes(const hydro *h)      // periodic axes whose ghost layers the stage kernels maintain
 {
     const long long cells = (long long)h->g.nx * h->g.ny * h->g.nz;
-    return fused_run(h) && h->g.ndim >= 2 && cells <= (1ll << 25) ? periodic_xy(h) : 0;    // (1D: periodic x keeps its fill)
+    return fused_run(h) && h->g.ndim >= 2 && cells <= (1ll << 25) ? periodic_xy(h) : 0;
 }
 
 int fill_axes(const hydro *h)      // axes ghost_fill_kernel fills before every stage
 {
     if (!fused_run(h)) return (1 << h->g.ndim) - 1;       // inactive axes have no ghost layers
+    if (h->g.ndim == 1) return 0;                         // the 1D kernel reads source cells, wrap included
     return periodic_xy(h) & ~wrap_axes(h);
 }
 
 int inkernel_axes(const hydro *h)  // axes whose boundary rule the fused kernels apply themselves
 {
+    if (fused_run(h) && h->g.ndim == 1) return 1;
     return fused_run(h) ? ((1 << h->g.ndim) - 1) & ~periodic_xy(h) : 0;
 }
 
@@ -581,7 +583,7 @@ int hydro_set_kernel_variant(hydro_t *h, int variant)
 {
     if (!h || variant < 0 || variant > 2) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0, 1 or 2%s%s");
     if (h->g.ndim == 1 && variant == 2)
-        return fail(HYDRO_ERR_ARG, "set_kernel_variant: a 1D run has variants 0 and 1 (its ghost cells always come from memory)%s%s");
+        return fail(HYDRO_ERR_ARG, "set_kernel_variant: a 1D run has variants 0 and 1%s%s");
     h->variant = variant;
     h->ghosts_valid = false;
     drop_graph(h);

@@ -10,10 +10,10 @@
 // work), three block barriers per tile.  With 130 / 171 fp64 instructions against 80 / 120 bytes
 // per cell and stage the 1D step is bound by HBM, not by the fp64 pipe: plain coalesced loads with
 // many resident blocks keep enough bytes in flight, so there is no TMA ring here: a block walks tiles of
-// 128 cells with the next tile's own values fetched one tile ahead, five blocks per SM.  Outflow and
-// reflecting ends are applied in the kernel (the ghost cells' source cells are read instead: three
-// launches per step); a periodic x keeps its ghost fill.  Same building blocks as the other stage
-// kernels (hydro_faces.cuh), so the verification build reproduces the oracle bit for bit.
+// 128 cells with the next tile's own values fetched one tile ahead, five blocks per SM.  The boundary
+// rule of x is applied in the kernel -- a ghost cell is read from its source cell (clamp / mirror / wrap):
+// three launches per step, the ghost cells in memory are never touched.  Same building blocks as the
+// other stage kernels (hydro_faces.cuh), so the verification build reproduces the oracle bit for bit.
 #pragma once
 #include "hydro_kernels.cuh"
 
@@ -39,10 +39,10 @@ stage_fused1d_kernel(Grid g, const double *__restrict__ Uin, const double *Uold,
     const double gamma = g.gamma, gm1 = g.gm1, igm1 = g.igm1, theta = g.theta;
     const double r = dev_dt ? dev_dt->dt / dx : dt_over_dx;
     const int ntile = (g.nx + F1T - 1) / F1T;
-    // inbc: the boundary rule of x is applied here (outflow / reflecting: a ghost cell takes the state of its
-    // source cell, normal momentum negated at a wall) and the ghost cells in memory are never read;
-    // otherwise (periodic x, or variant 0's ghost fill) they are read from memory.  Cells past the high
-    // ghost layer are never used by an active cell: clamped to stay addressable.
+    // inbc: the boundary rule of x is applied here (a ghost cell takes the state of its source cell: nearest
+    // cell / mirror image with the normal momentum negated / periodic image) and the ghost cells in
+    // memory are never read; otherwise they are read from memory.  Cells past the high ghost layer
+    // are never used by an active cell: clamped to stay addressable.
     auto load_plain = [&](const double *U, int ii, double out[5]) {
         const long long c = c0 + min(ii, g.nx + NG - 1);
 #pragma unroll

@@ -32,7 +32,7 @@ CASES = [
     (1, (257, 1, 1), (0.01, 1.0, 1.0), (OUT, OUT, OUT, OUT, OUT, OUT)),
     (1, (64, 1, 1), (0.3, 1.0, 1.0), (REF, OUT, OUT, OUT, OUT, OUT)),
     (1, (200001, 1, 1), (1e-5, 1.0, 1.0), (OUT, REF, OUT, OUT, OUT, OUT)),    # fused 1D kernel: more tiles than resident blocks
-    (1, (1000, 1, 1), (1e-3, 1.0, 1.0), (PER, PER, OUT, OUT, OUT, OUT)),       # periodic x keeps its ghost fill
+    (1, (1000, 1, 1), (1e-3, 1.0, 1.0), (PER, PER, OUT, OUT, OUT, OUT)),       # periodic x: wrapped source cells
     (1, (2, 1, 1), (0.3, 1.0, 1.0), (PER, PER, OUT, OUT, OUT, OUT)),
     (2, (70, 37, 1), (0.02, 0.02, 1.0), (OUT, REF, PER, PER, OUT, OUT)),
     (2, (33, 5, 1), (0.1, 0.031, 1.0), (PER, PER, REF, OUT, OUT, OUT)),
@@ -145,17 +145,17 @@ def test_create_nd_status_codes():
     g = Hydro(8, 1, 1, 1.4, 0.1, (0,) * 6, ndim=1, dxyz=(0.1, 0.2, 0.1))
     g.set_kernel_variant(0); g.set_kernel_variant(1)       # 1D runs: simple or fused 1D kernel
     with pytest.raises(HydroError):
-        g.set_kernel_variant(2)                            # (their ghost cells always come from memory)
+        g.set_kernel_variant(2)                            # (variant 2 is the 2D / 3D cross-check)
     with pytest.raises(HydroError):
         g.set_tiling(16, 4)
 
 
 @pytest.mark.gpu
 def test_1d_launches_per_step():
-    """The fused 1D kernel applies outflow and reflecting ends itself (three launches per step: start of
-    step, two stages); a periodic x keeps its ghost fill (four); the simple kernel always fills (four)."""
+    """The fused 1D kernel applies every boundary kind itself (three launches per step: start of step, two
+    stages); the simple kernel has its ghost cells filled in memory before each stage (four)."""
     from paper_1812_07977_b200.binding import Hydro
-    for bc0, variant, want in ((OUT, 1, 3), (REF, 1, 3), (PER, 1, 4), (OUT, 0, 4)):
+    for bc0, variant, want in ((OUT, 1, 3), (REF, 1, 3), (PER, 1, 3), (OUT, 0, 4)):
         bc = (bc0, bc0, OUT, OUT, OUT, OUT)
         g = Hydro(500, 1, 1, 1.4, 1.0 / 500, bc, ndim=1)
         g.set_kernel_variant(variant)
