@@ -110,3 +110,19 @@ def test_tiling_partition_balances_the_paper_sizes(libs):
         remainder = rounds * (lzr + 1.25)
         assert abs(primary - remainder) <= 0.15 * primary          # the two sides finish together
         assert primary < 1.06 * (n * tiles / 148 + 1.25)            # within 6 % of a perfect split
+
+
+def test_committed_ncu_capture_is_of_the_committed_sources():
+    """bench.py's roofline.traffic comes from profiles/traffic.txt, which names the sources (hash of
+    csrc/) its ncu capture was taken from; bench.py refuses a capture of other sources.  The committed
+    pair must match, so that the bench line carries a measured traffic figure."""
+    import sys
+    sys.path.insert(0, ROOT)
+    import bench
+    p = os.path.join(ROOT, "profiles", "traffic.txt")
+    if not os.path.exists(p):
+        pytest.skip("no committed capture")
+    kv = dict(ln.split() for ln in open(p) if len(ln.split()) == 2 and not ln.startswith("#"))
+    assert kv["csrc_sha256"] == bench.csrc_sha256(), "re-capture profiles/ after changing csrc/"
+    t = bench.load_traffic(3)
+    assert t["dram"] and abs(t["dram"] / (200.0 * 256 ** 3) - 1.0) < 0.1      # within 10 % of the algorithmic bytes
