@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 SOURCES = ["hydro_api.cu"]
 HEADERS = ["hydro_math.cuh", "hydro_math_fast.cuh", "hydro_faces.cuh", "hydro_kernels.cuh", "hydro_stage_fused.cuh",
            "hydro_stage_fused_kernel.cuh", "hydro_stage_fused_plan.cuh", "hydro_stage_fused2d.cuh",
-           "hydro_stage_fused1d.cuh",
+           "hydro_stage_fused1d.cuh", "hydro_stage_warp2d.cuh",
            "hydro_tma.cuh"]
 LIB = os.path.join(HERE, "libhydro_b200.so")
 LIB_VERIFY = os.path.join(HERE, "libhydro_b200_verify.so")

@@ -7,6 +7,7 @@
 #include "hydro_stage_fused.cuh"
 #include "hydro_stage_fused2d.cuh"
 #include "hydro_stage_fused1d.cuh"
+#include "hydro_stage_warp2d.cuh"
 
 #include <atomic>
 #include <cmath>
@@ -68,6 +69,7 @@ struct hydro {
     double t = 0.0;
     long long step = 0;
     int variant = 1;
+    int w2rows = 0;                 // warp-column 2D kernel: rows per chunk (0: not chosen yet)
     bool graph_replay = true;       // hydro_set_graph_replay
     int ty_req = 0, lz_req = 0;     // hydro_set_tiling (0 = chosen by the library)
     FusedPlan plan;                 // launch geometry / TMA descriptors of the fused kernel
@@ -170,6 +172,7 @@ int periodic_xy(const hydro *h)
 }
 
 bool fused_run(const hydro *h) { return h->variant == 1; }
+bool warp2d_run(const hydro *h) { return h->g.ndim == 2 && h->variant == 3; }   // every boundary applied on the way in
 
 int wrap_axes(const hydro *h)      // periodic axes whose ghost layers the stage kernels maintain
 {
@@ -179,6 +182,7 @@ int wrap_axes(const hydro *h)      // periodic axes whose ghost layers the stage
 
 int fill_axes(const hydro *h)      // axes ghost_fill_kernel fills before every stage
 {
+    if (warp2d_run(h)) return 0;
     if (!fused_run(h)) return (1 << h->g.ndim) - 1;       // inactive axes have no ghost layers
     if (h->g.ndim == 1) return 0;                         // the 1D kernel reads source cells, wrap included
     return periodic_xy(h) & ~wrap_axes(h);
@@ -264,6 +268,17 @@ int launch_stage(hydro *h, const double *in, const double *old, double *out, dou
         cudaError_t e1 = launch_stage_fused1d<STAGE>(g, in, old, out, r, dd, h->dx, red, inkernel_axes(h) & 1, h->stream);
         g_launches.fetch_add(1, std::memory_order_relaxed);
         if (e1 != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_fused1d: %s%s", cudaGetErrorString(e1));
+        return HYDRO_OK;
+    }
+    if (warp2d_run(h)) {                      // warp-column 2D kernel
+        if (!h->w2rows) {
+            int nsm = 148, dev = 0;
+            if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+            h->w2rows = warp2d_choose_rows(g, nsm);
+        }
+        cudaError_t ew = launch_stage_warp2d<STAGE>(g, in, old, out, r, dd, h->dx, red, h->w2rows, h->stream);
+        g_launches.fetch_add(1, std::memory_order_relaxed);
+        if (ew != cudaSuccess) return fail(HYDRO_ERR_CUDA, "launch stage_warp2d: %s%s", cudaGetErrorString(ew));
         return HYDRO_OK;
     }
     const int inbc = inkernel_axes(h);
@@ -581,7 +596,9 @@ int hydro_set_limiter_theta(hydro_t *h, double theta)
 
 int hydro_set_kernel_variant(hydro_t *h, int variant)
 {
-    if (!h || variant < 0 || variant > 2) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0, 1 or 2%s%s");
+    if (!h || variant < 0 || variant > 3) return fail(HYDRO_ERR_ARG, "set_kernel_variant: 0, 1, 2 or 3%s%s");
+    if (variant == 3 && h->g.ndim != 2)
+        return fail(HYDRO_ERR_ARG, "set_kernel_variant: variant 3 is the warp-column kernel of 2D runs%s%s");
     if (h->g.ndim == 1 && variant == 2)
         return fail(HYDRO_ERR_ARG, "set_kernel_variant: a 1D run has variants 0 and 1%s%s");
     h->variant = variant;

@@ -48,7 +48,7 @@ CASES = [
 @pytest.mark.parametrize("ndim,shape,dxyz,bc", CASES)
 def test_nd_runs_bit_identical_on_verification_build(ndim, shape, dxyz, bc):
     U = inputs.random_state(*shape, seed=sum(shape) + ndim, vamp=0.5)
-    variants = (1, 2, 0) if ndim >= 2 else (1, 0)
+    variants = {1: (1, 0), 2: (3, 1, 2, 0), 3: (1, 2, 0)}[ndim]
     for variant in variants:
         g, c = _pair(shape, ndim, dxyz, bc, variant=variant)
         if ndim == 2 and variant == 2:
@@ -139,11 +139,14 @@ def test_create_nd_status_codes():
     with pytest.raises(HydroError):
         Hydro(8, 8, 1, 1.4, 0.1, (0,) * 6, ndim=2, dxyz=(0.1, -0.1, 0.1))
     g = Hydro(8, 8, 1, 1.4, 0.1, (0,) * 6, ndim=2, dxyz=(0.1, 0.2, 0.1))
+    g.set_kernel_variant(3)                                # warp-column kernel: 2D runs only
     g.set_kernel_variant(1); g.set_tiling(16, 4)
     with pytest.raises(HydroError):
         g.set_tiling(8, 4)                                 # 2D runs use 32 x 16 tiles
     g = Hydro(8, 1, 1, 1.4, 0.1, (0,) * 6, ndim=1, dxyz=(0.1, 0.2, 0.1))
     g.set_kernel_variant(0); g.set_kernel_variant(1)       # 1D runs: simple or fused 1D kernel
+    with pytest.raises(HydroError):
+        g.set_kernel_variant(3)
     with pytest.raises(HydroError):
         g.set_kernel_variant(2)                            # (variant 2 is the 2D / 3D cross-check)
     with pytest.raises(HydroError):
