@@ -67,6 +67,9 @@ enum {
  * ideal gas with adiabatic index gamma (R1).
  *   bc[6]: HYDRO_BC_* for faces xlo,xhi,ylo,yhi,zlo,zhi (host pointer, copied).
  * Defaults: CFL 0.7, limiter theta 1.4.
+ * Performance note: the stage kernels tile x in units of 32 cells and y in units of 8 or 16 and march
+ * along z, so a grid with one short or awkward extent (33, 100) runs best with that extent as nz (the
+ * scheme is symmetric under relabelling of the axes).
  * HYDRO_ERR_ARG if nx,ny,nz < 2, gamma <= 1, dx <= 0 or non-finite, unknown bc value,
  * periodic on only one face of an axis, or a NULL pointer.  *out is NULL on failure. */
 int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6],
