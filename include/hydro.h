@@ -237,7 +237,8 @@ int hydro_set_graph_replay(hydro_t *h, int enable);
  * runs).  3 = 2D runs only: the "warp column" kernel -- a warp owns a 32-lane strip and marches down y
  * with the y direction in registers and the x direction exchanged by warp shuffles (no shared memory,
  * no barriers, every boundary kind applied on the way in); within 2 % of variant 1 on large grids,
- * 10-15 % faster around 1024^2 - 2048^2, slower below 768^2. */
+ * 10-15 % faster around 1024^2 - 2048^2, slower below 768^2; the default of 2D
+ * runs of 2^20 cells and more. */
 int hydro_set_kernel_variant(hydro_t *h, int variant);
 /* Measurement hooks (bench.py): when enabled, every kernel launch of this handle is bracketed by
  * CUDA events on the handle's stream.  hydro_get_kernel_time synchronises and returns the summed

@@ -504,6 +504,9 @@ int hydro_create_nd(int ndim, const int n[3], const double d[3], double gamma, c
     for (int f = 0; f < 6; ++f) g.bc[f] = f < 2 * ndim ? bc[f] : HYDRO_BC_OUTFLOW;
     g.gamma = gamma; g.gm1 = gamma - 1.0; g.igm1 = 1.0 / g.gm1; g.theta = 1.4;
     h->dx = d[0]; h->cfl = 0.7;
+    // 2D runs of a megacell and more default to the warp-column kernel (never slower there, 10-15 % faster
+    // around 1024^2 - 2048^2; smaller grids are better off with the tiled kernel: DESIGN.md section 6.4)
+    if (ndim == 2 && (long long)n[0] * n[1] >= (1ll << 20)) h->variant = 3;
     h->dmin = d[0];
     for (int a = 0; a < 3; ++a) {
         h->dxyz[a] = a < ndim ? d[a] : d[0];

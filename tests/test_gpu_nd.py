@@ -169,3 +169,29 @@ def test_1d_launches_per_step():
         g.run_steps(5)
         assert g.launch_count() - n0 == 5 * want, (bc0, variant, g.launch_count() - n0)
         g.close()
+
+
+@pytest.mark.gpu
+def test_2d_variants_agree_bitwise_on_a_large_grid():
+    """2D runs of a megacell and more default to the warp-column kernel (variant 3).  On a grid of that
+    size -- many strips, many chunks of rows, non-cubic cells, mixed boundaries -- the verification build
+    gives the same bits with the warp-column, the tiled and the simple kernel (each of which equals the
+    oracle on the small grids above), and the production build stays within the one-step bar of it."""
+    import torch
+    from paper_1812_07977_b200.binding import Hydro
+    nx, ny = 1100, 1000
+    bc = (REF, OUT, PER, PER, OUT, OUT)
+    U = torch.from_numpy(inputs.random_state(nx, ny, 1, seed=77, vamp=0.4)).cuda()
+    out = {}
+    for variant in (None, 1, 0):
+        g = Hydro(nx, ny, 1, 1.4, 1.0 / nx, bc, verify=True, ndim=2, dxyz=(1.0 / nx, 1.3 / nx, 1.0))
+        if variant is not None:
+            g.set_kernel_variant(variant)
+        g.set_state(U); g.run_steps(3)
+        out[variant] = g.get_state()
+        g.close()
+    assert np.array_equal(out[None], out[1]) and np.array_equal(out[None], out[0])
+    g = Hydro(nx, ny, 1, 1.4, 1.0 / nx, bc, verify=False, ndim=2, dxyz=(1.0 / nx, 1.3 / nx, 1.0))
+    g.set_state(U); g.run_steps(3)
+    assert_one_step_bar(g.get_state(), out[None], tol=6e-14)
+    g.close()
