@@ -68,8 +68,8 @@ enum {
  *   bc[6]: HYDRO_BC_* for faces xlo,xhi,ylo,yhi,zlo,zhi (host pointer, copied).
  * Defaults: CFL 0.7, limiter theta 1.4.
  * Performance note: the stage kernels tile x in units of 32 cells and y in units of 8 or 16 and march
- * along z, so a grid with one short or awkward extent (33, 100) runs best with that extent as nz (the
- * scheme is symmetric under relabelling of the axes).
+ * along z, so a grid with one awkward extent (33) is cheapest with that extent as nz; the library holds
+ * such a run with its axes relabelled by itself (hydro_get_axis_order below).
  * HYDRO_ERR_ARG if nx,ny,nz < 2, gamma <= 1, dx <= 0 or non-finite, unknown bc value,
  * periodic on only one face of an axis, or a NULL pointer.  *out is NULL on failure. */
 int hydro_create(int nx, int ny, int nz, double gamma, double dx, const int bc[6],
@@ -227,6 +227,13 @@ int hydro_get_tiling(hydro_t *h, int *tile_rows, int *planes_per_chunk, long lon
 int hydro_tiling_partition(int nx, int ny, int nz, int tile_rows, int planes_per_chunk, int sms, int kb, int ke,
                            int out[5]);
 int hydro_set_graph_replay(hydro_t *h, int enable);
+/* The library may hold a 3D run of cubic cells with its axes relabelled when the launch-geometry cost
+ * model says another order is at least 12 % cheaper (a grid 33 cells wide costs two 32-wide tile columns;
+ * as nz it costs nothing): the scheme is symmetric under relabelling, and only the copies in and out of
+ * the handle know.  Every call keeps the caller's axis order; hydro_get_axis_order reports the internal
+ * axis of the caller's axes x, y, z (0, 1, 2 = not relabelled).  hydro_get_padded is not available on
+ * a relabelled handle (HYDRO_ERR_ARG). */
+int hydro_get_axis_order(hydro_t *h, int order[3]);
 /* Select the stage-kernel implementation:
  * 0 = reference-structured simple kernel (one thread per
  * cell, everything recomputed, ghost layers filled in memory before each substep); 1 = fused tiled

@@ -20,7 +20,7 @@ SYMBOLS = ["hydro_create", "hydro_create_nd", "hydro_set_state", "hydro_cfl_dt",
            "hydro_get_state", "hydro_destroy", "hydro_set_cfl", "hydro_set_limiter_theta",
            "hydro_get_time", "hydro_max_signal_speed", "hydro_set_stream", "hydro_set_allocator",
            "hydro_run_steps", "hydro_ghost_fill", "hydro_get_padded", "hydro_set_kernel_variant",
-           "hydro_set_tiling", "hydro_get_tiling", "hydro_tiling_partition", "hydro_set_graph_replay",
+           "hydro_set_tiling", "hydro_get_tiling", "hydro_tiling_partition", "hydro_set_graph_replay", "hydro_get_axis_order",
            "hydro_create_slab", "hydro_substep", "hydro_halo_count", "hydro_halo_pack",
            "hydro_halo_unpack", "hydro_halo_push", "hydro_state_base", "hydro_smax_device",
            "hydro_reduce_smax", "hydro_host_alloc", "hydro_update_device", "hydro_update_host",
@@ -80,6 +80,7 @@ def load_library(verify=False):
     L.hydro_set_tiling.argtypes = [vp, C.c_int, C.c_int]
     L.hydro_get_tiling.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.POINTER(C.c_longlong)]
     L.hydro_set_graph_replay.argtypes = [vp, C.c_int]
+    L.hydro_get_axis_order.argtypes = [vp, C.POINTER(C.c_int)]
     L.hydro_tiling_partition.argtypes = [C.c_int] * 8 + [C.POINTER(C.c_int)]
     L.hydro_create_slab.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.POINTER(C.c_int),
                                     C.c_int, C.c_int, C.POINTER(vp), C.POINTER(C.c_int), C.POINTER(C.c_int)]
@@ -253,6 +254,11 @@ class Hydro:
         self._chk(self._L.hydro_get_tiling(self._h, C.byref(ty), C.byref(lz), C.byref(nb)),
                   "hydro_get_tiling")
         return {"tile": [32, ty.value], "planes_per_chunk": lz.value, "blocks": nb.value}
+
+    def get_axis_order(self):
+        o = (C.c_int * 3)()
+        self._chk(self._L.hydro_get_axis_order(self._h, o), "hydro_get_axis_order")
+        return list(o)
 
     def set_graph_replay(self, enable):
         self._chk(self._L.hydro_set_graph_replay(self._h, int(bool(enable))), "hydro_set_graph_replay")

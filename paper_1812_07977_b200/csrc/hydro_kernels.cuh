@@ -344,21 +344,33 @@ __global__ void halo_kernel(Grid g, double *U, double *other, int K0, int Kd, lo
 // pack / unpack between the packed [5][nz][ny][nx] layout and the padded state (device side;
 // host pointers go through cudaMemcpy3D in the API layer).
 // ------------------------------------------------------------------------------------------
+// The library may hold a 3D run with its axes relabelled (hydro_api.cu, "axis order"): the caller's axis a is
+// the internal axis ax[a], the caller's variable v the internal variable var[v] (the momentum components
+// follow their axes).  n = the caller's extents.  Identity for every other handle.
+struct AxisMap {
+    int n[3];
+    int ax[3];
+    int var[NVAR];
+};
+
 template <bool TO_PADDED>
-__global__ void repack_kernel(Grid g, double *padded, double *packed, unsigned fields)
+__global__ void repack_kernel(Grid g, AxisMap m, double *padded, double *packed, unsigned fields)
 {
-    const long long nact = (long long)g.nx * g.ny * g.nz;
+    const long long nact = (long long)m.n[0] * m.n[1] * m.n[2];
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < nact;
          t += (long long)gridDim.x * blockDim.x) {
-        const int i = (int)(t % g.nx);
-        const long long jk = t / g.nx;
-        const int j = (int)(jk % g.ny), k = (int)(jk / g.ny);
+        const int iu = (int)(t % m.n[0]);
+        const long long jk = t / m.n[0];
+        const int ju = (int)(jk % m.n[1]), ku = (int)(jk / m.n[1]);
+        const int i = m.ax[0] == 0 ? iu : (m.ax[1] == 0 ? ju : ku);
+        const int j = m.ax[0] == 1 ? iu : (m.ax[1] == 1 ? ju : ku);
+        const int k = m.ax[0] == 2 ? iu : (m.ax[1] == 2 ? ju : ku);
         const long long c = cell0(g, i, j, k);
 #pragma unroll
         for (int v = 0; v < NVAR; ++v) {
             if (!(fields >> v & 1u)) continue;               // selected fields only
-            if (TO_PADDED) padded[v * g.sv + c] = packed[v * nact + t];
-            else packed[v * nact + t] = padded[v * g.sv + c];
+            if (TO_PADDED) padded[m.var[v] * g.sv + c] = packed[v * nact + t];
+            else packed[v * nact + t] = padded[m.var[v] * g.sv + c];
         }
     }
 }
