@@ -254,6 +254,33 @@ int hydro_set_kernel_variant(hydro_t *h, int variant);
  * the step has no ghost fill to carry them), 4 stand-alone CFL reduction. */
 int hydro_set_profiling(hydro_t *h, int enable);
 int hydro_get_kernel_time(hydro_t *h, int which, double *ms, long long *count);
+/* ---- allocation-free entry point ---------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid it): Algorithm 1 line 5, "ComputeTimeStep" -- the reduction
+ * max(|v| + c_s) over the cells of a packed state (R8; the same arithmetic as hydro_max_signal_speed) --
+ * without a handle and without any allocation: no cudaMalloc, cudaFree or allocating library routine is
+ * called.  The scratch of the reduction (one partial maximum per block of 2048 cells and a ticket) is a
+ * file-scope device array of HYDRO_NOALLOC_SCRATCH_BYTES (1 MiB + 256 B) that every GPU loading this
+ * library holds until the process exits; its capacity sets the limit HYDRO_NOALLOC_MAX_CELLS = 2^27
+ * cells (512^3, the largest configuration).
+ *   U_dev:    DEVICE pointer (current device), packed double U[5][ncells] (rho, m_x, m_y, m_z, E; the
+ *             layout of hydro_get_state with ncells = nx*ny*nz); read only, the caller keeps ownership.
+ *   smax_dev: DEVICE pointer to one double, receives max(|v| + c_s) (0 if no cell has a positive speed).
+ *   flag_dev: DEVICE pointer to one int, receives 1 if any cell has rho <= 0, p <= 0 or a non-finite
+ *             speed (HYDRO_ERR_UNPHYSICAL's condition), else 0.
+ *   cuda_stream: the cudaStream_t to enqueue on (NULL = default stream).  Asynchronous: the outputs are
+ *             valid once the stream has run the call; the time step is (cfl/ndim) * min_d(d[a]) / *smax_dev.
+ * Every call on a device shares the one scratch array, which keeps the last call's contents (the call
+ * clears what must start at zero itself): calls that overlap on the GPU -- two streams, two threads --
+ * race on it and give wrong results; calls on one stream, or otherwise ordered, are safe.  The first call
+ * on a device looks up the array's address (cudaGetSymbolAddress); make that call outside graph capture.
+ * HYDRO_ERR_ARG (before any CUDA call) for a NULL pointer, ncells < 1, ncells > HYDRO_NOALLOC_MAX_CELLS
+ * (use a handle and hydro_max_signal_speed for larger states) or gamma <= 1; HYDRO_ERR_ARG for a host
+ * pointer; HYDRO_ERR_CUDA if a CUDA call fails.  Not counted by hydro_get_kernel_time. */
+#define HYDRO_NOALLOC_MAX_CELLS 134217728LL
+#define HYDRO_NOALLOC_SCRATCH_BYTES 1048832
+int hydro_max_signal_speed_noalloc(const double *U_dev, long long ncells, double gamma,
+                                   double *smax_dev, int *flag_dev, void *cuda_stream);
 /* Number of kernels this library has launched since load (for bench.py's gpu_launches). */
 long long hydro_launch_count(void);
 /* 1 if this library was compiled with -fmad=false (verification build), else 0. */

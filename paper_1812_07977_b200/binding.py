@@ -24,7 +24,7 @@ SYMBOLS = ["hydro_create", "hydro_create_nd", "hydro_set_state", "hydro_cfl_dt",
            "hydro_create_slab", "hydro_substep", "hydro_halo_count", "hydro_halo_pack",
            "hydro_halo_unpack", "hydro_halo_push", "hydro_state_base", "hydro_smax_device",
            "hydro_reduce_smax", "hydro_host_alloc", "hydro_update_device", "hydro_update_host",
-           "hydro_transfer_sync",
+           "hydro_transfer_sync", "hydro_max_signal_speed_noalloc",
            "hydro_set_profiling", "hydro_get_kernel_time", "hydro_launch_count",
            "hydro_is_verification_build", "hydro_last_error"]
 
@@ -96,6 +96,7 @@ def load_library(verify=False):
     L.hydro_update_device.argtypes = [vp, C.c_uint, vp]
     L.hydro_update_host.argtypes = [vp, C.c_uint, vp]
     L.hydro_transfer_sync.argtypes = [vp]
+    L.hydro_max_signal_speed_noalloc.argtypes = [vp, C.c_longlong, C.c_double, vp, vp, vp]
     L.hydro_set_profiling.argtypes = [vp, C.c_int]
     L.hydro_get_kernel_time.argtypes = [vp, C.c_int, _dp, C.POINTER(C.c_longlong)]
     L.hydro_launch_count.restype = C.c_longlong
@@ -123,6 +124,31 @@ def tiling_partition(nx, ny, nz, tile_rows, planes_per_chunk=0, sms=148, kb=0, k
             k0 = km + (z - nprim) * lzr; k1 = min(k0 + lzr, ke)
         layers.append((k0, k1))
     return layers, (lz, km, nprim, lzr, nlayer)
+
+
+NOALLOC_MAX_CELLS = 1 << 27          # HYDRO_NOALLOC_MAX_CELLS
+
+
+def max_signal_speed_noalloc(U, gamma, smax_out, flag_out, stream=None, verify=False):
+    """hydro_max_signal_speed_noalloc: max(|v| + c_s) of a packed CUDA tensor U[5][...] into the CUDA
+    tensors smax_out (one float64) and flag_out (one int32), enqueued on `stream` (a cudaStream_t as an
+    int; default: torch's current stream).  Allocates nothing; asynchronous."""
+    import torch
+    L = load_library(verify)
+    if not (isinstance(U, torch.Tensor) and U.is_cuda and U.dtype == torch.float64 and U.is_contiguous()
+            and U.dim() >= 1 and U.shape[0] == 5):
+        raise ValueError("need a contiguous float64 CUDA tensor U[5][...]")
+    if not (smax_out.is_cuda and smax_out.dtype == torch.float64 and smax_out.numel() == 1
+            and flag_out.is_cuda and flag_out.dtype == torch.int32 and flag_out.numel() == 1):
+        raise ValueError("need one float64 and one int32 CUDA element for the outputs")
+    if stream is None:
+        stream = torch.cuda.current_stream(U.device).cuda_stream
+    with torch.cuda.device(U.device):
+        rc = L.hydro_max_signal_speed_noalloc(C.c_void_p(U.data_ptr()), U.numel() // 5, float(gamma),
+                                              C.c_void_p(smax_out.data_ptr()), C.c_void_p(flag_out.data_ptr()),
+                                              C.c_void_p(int(stream)))
+    if rc:
+        raise HydroError(rc, "hydro_max_signal_speed_noalloc", L.hydro_last_error().decode())
 
 
 def use_torch_allocator(L, enable=True):

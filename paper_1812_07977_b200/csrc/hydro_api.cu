@@ -1160,3 +1160,170 @@ int hydro_get_time(hydro_t *h, double *t, long long *step)
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// Allocation-free entry point: hydro_max_signal_speed_noalloc (include/hydro.h).
+// The CFL reduction (A8) of a packed device state for callers that cannot call cudaMalloc (CUDA graph
+// capture, tight serving loops, harnesses that forbid it).  No handle, no cudaMalloc / cudaFree, no
+// allocating library routine: the scratch of the reduction -- one partial maximum per block and the
+// ticket that finds the last block -- lives in a file-scope device array of fixed size, which every
+// GPU that loads this library holds until the process exits.
+//
+// In host code `g_noalloc_scratch` is a host-side stand-in for the device array, not a device address:
+// the host asks cudaGetSymbolAddress for the address once per device, with that device current, and
+// passes it to the kernel.  Every call on a device shares the array, which keeps the last call's
+// contents: the ticket is cleared at the start of each call, partials beyond the launch's own blocks
+// are never read.  Calls that overlap on the GPU (two streams, two threads) race on it.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+constexpr int NOALLOC_THREADS = 256;
+constexpr int NOALLOC_CELLS_PER_THREAD = 8;
+constexpr long long NOALLOC_CELLS_PER_BLOCK = (long long)NOALLOC_THREADS * NOALLOC_CELLS_PER_THREAD;   // 2048
+constexpr long long NOALLOC_MAX_BLOCKS = HYDRO_NOALLOC_MAX_CELLS / NOALLOC_CELLS_PER_BLOCK;            // 65536
+constexpr size_t NOALLOC_HEADER_BYTES = 256;      // ticket (4 bytes used); the partials start 256-byte aligned
+
+struct NoallocPartial { double smax; int bad; int pad; };                                               // 16 bytes
+
+constexpr size_t NOALLOC_SCRATCH_BYTES = NOALLOC_HEADER_BYTES + (size_t)NOALLOC_MAX_BLOCKS * sizeof(NoallocPartial);
+static_assert(NOALLOC_SCRATCH_BYTES == HYDRO_NOALLOC_SCRATCH_BYTES, "hydro.h states the size of the scratch array");
+static_assert(NOALLOC_MAX_BLOCKS * NOALLOC_CELLS_PER_BLOCK == HYDRO_NOALLOC_MAX_CELLS, "whole blocks");
+
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_SCRATCH_BYTES];
+
+// One block = one chunk of 2048 cells of the packed state U[5][ncells] (coalesced: consecutive threads,
+// consecutive cells); the block's maximum and unphysical flag go to partial[blockIdx.x]; the block that
+// draws the last ticket folds the partials of this launch in a fixed order and writes the two outputs.
+// The maximum does not depend on the order, so the result is deterministic and equal to the atomicMax
+// form of cfl_reduce_kernel.
+__global__ void __launch_bounds__(NOALLOC_THREADS)
+cfl_reduce_noalloc_kernel(const double *__restrict__ U, long long ncells, double gamma, double gm1,
+                          unsigned char *scratch, double *smax_out, int *flag_out)
+{
+    unsigned *ticket = reinterpret_cast<unsigned *>(scratch);
+    NoallocPartial *partial = reinterpret_cast<NoallocPartial *>(scratch + NOALLOC_HEADER_BYTES);
+    __shared__ double wmax[NOALLOC_THREADS / 32];
+    __shared__ int wbad[NOALLOC_THREADS / 32];
+    __shared__ int is_last;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+
+    double s = 0.0;
+    int bad = 0;
+    const long long first = (long long)blockIdx.x * NOALLOC_CELLS_PER_BLOCK + threadIdx.x;
+#pragma unroll
+    for (int q = 0; q < NOALLOC_CELLS_PER_THREAD; ++q) {
+        const long long c = first + (long long)q * NOALLOC_THREADS;
+        if (c < ncells) {
+            const double v = cell_signal_speed(U[c], U[ncells + c], U[2 * ncells + c], U[3 * ncells + c],
+                                               U[4 * ncells + c], gamma, gm1, bad);
+            s = v > s ? v : s;                 // NaN never wins; it is reported through `bad`
+        }
+    }
+    auto fold = [&]() {                        // block-wide maximum / or into thread 0
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double other = __shfl_xor_sync(0xffffffffu, s, o);
+            s = other > s ? other : s;
+            bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+        }
+        if (lane == 0) { wmax[wid] = s; wbad[wid] = bad; }
+        __syncthreads();
+        if (wid == 0) {
+            s = lane < NOALLOC_THREADS / 32 ? wmax[lane] : 0.0;
+            bad = lane < NOALLOC_THREADS / 32 ? wbad[lane] : 0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                const double other = __shfl_xor_sync(0xffffffffu, s, o);
+                s = other > s ? other : s;
+                bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+            }
+        }
+    };
+    fold();
+    if (threadIdx.x == 0) {
+        partial[blockIdx.x].smax = s;
+        partial[blockIdx.x].bad = bad;
+        __threadfence();                       // the partial is visible before the ticket is drawn
+        is_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    s = 0.0;
+    bad = 0;
+    for (unsigned b = threadIdx.x; b < gridDim.x; b += NOALLOC_THREADS) {
+        const double v = __ldcg(&partial[b].smax);
+        bad |= __ldcg(&partial[b].bad);
+        s = v > s ? v : s;
+    }
+    __syncthreads();                           // wmax / wbad are reused
+    fold();
+    if (threadIdx.x == 0) {
+        *smax_out = s;
+        *flag_out = bad ? 1 : 0;
+        *ticket = 0u;                          // left clean for the next call (which clears it again)
+    }
+}
+
+// Device address of the scratch array, looked up once per device (set-up) with that device current.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::atomic<unsigned char *> g_noalloc_ptr[NOALLOC_MAX_DEVICES];
+
+int noalloc_scratch(unsigned char **out)
+{
+    int dev = -1;
+    CUDA_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= NOALLOC_MAX_DEVICES)
+        return fail(HYDRO_ERR_CUDA, "max_signal_speed_noalloc: device ordinal beyond 63%s%s");
+    unsigned char *p = g_noalloc_ptr[dev].load(std::memory_order_acquire);
+    if (!p) {
+        // `dev` is current: the address returned is that of this device's copy of the array
+        CUDA_TRY(cudaGetSymbolAddress((void **)&p, g_noalloc_scratch));
+        if (!p) return fail(HYDRO_ERR_CUDA, "max_signal_speed_noalloc: cudaGetSymbolAddress returned NULL%s%s");
+        g_noalloc_ptr[dev].store(p, std::memory_order_release);   // two threads racing store the same address
+    }
+    *out = p;
+    return HYDRO_OK;
+}
+
+// HYDRO_ERR_ARG unless `p` is memory the current device can dereference as its own (device or managed)
+int noalloc_device_pointer(const void *p, const char *what)
+{
+    cudaPointerAttributes at;
+    const cudaError_t e = cudaPointerGetAttributes(&at, p);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(HYDRO_ERR_CUDA, "max_signal_speed_noalloc: cudaPointerGetAttributes(%s): %s", what, cudaGetErrorString(e));
+    }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return fail(HYDRO_ERR_ARG, "max_signal_speed_noalloc: %s is not a device pointer%s", what);
+    return HYDRO_OK;
+}
+
+}  // namespace
+
+extern "C" int hydro_max_signal_speed_noalloc(const double *U_dev, long long ncells, double gamma,
+                                              double *smax_dev, int *flag_dev, void *cuda_stream)
+{
+    // argument checks first: none of them needs a device
+    if (!U_dev || !smax_dev || !flag_dev) return fail(HYDRO_ERR_ARG, "max_signal_speed_noalloc: NULL pointer%s%s");
+    if (ncells < 1) return fail(HYDRO_ERR_ARG, "max_signal_speed_noalloc: ncells must be at least 1%s%s");
+    if (ncells > HYDRO_NOALLOC_MAX_CELLS)
+        return fail(HYDRO_ERR_ARG, "max_signal_speed_noalloc: ncells exceeds HYDRO_NOALLOC_MAX_CELLS = 134217728 (512^3), "
+                                   "the capacity of the static scratch array; use a handle (hydro_max_signal_speed)%s%s");
+    if (!(gamma > 1.0) || !std::isfinite(gamma)) return fail(HYDRO_ERR_ARG, "max_signal_speed_noalloc: gamma must be > 1%s%s");
+    int rc;
+    if ((rc = noalloc_device_pointer(U_dev, "U_dev"))) return rc;
+    if ((rc = noalloc_device_pointer(smax_dev, "smax_dev"))) return rc;
+    if ((rc = noalloc_device_pointer(flag_dev, "flag_dev"))) return rc;
+    unsigned char *scratch = nullptr;
+    if ((rc = noalloc_scratch(&scratch))) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    // what must start at zero: the ticket (the header); a memset node under capture, allocates nothing
+    CUDA_TRY(cudaMemsetAsync(scratch, 0, NOALLOC_HEADER_BYTES, stream));
+    const unsigned blocks = (unsigned)((ncells + NOALLOC_CELLS_PER_BLOCK - 1) / NOALLOC_CELLS_PER_BLOCK);
+    cfl_reduce_noalloc_kernel<<<blocks, NOALLOC_THREADS, 0, stream>>>(U_dev, ncells, gamma, gamma - 1.0, scratch,
+                                                                     smax_dev, flag_dev);
+    LAUNCH_CHECK("cfl_reduce_noalloc");
+    return HYDRO_OK;
+}
