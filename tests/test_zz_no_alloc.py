@@ -151,6 +151,32 @@ def test_allocates_nothing_and_rejects_host_pointers():
     assert rc == 1 and b"not a device pointer" in L.hydro_last_error()
 
 
+@pytest.mark.gpu
+def test_captured_into_a_cuda_graph_and_replayed():
+    """What the entry point is for: captured into a CUDA graph (torch's capture runs in the mode in which
+    a cudaMalloc anywhere in the process invalidates the capture), then replayed on changing inputs.  The
+    first call on the device -- the set-up that looks up the scratch address -- is made outside capture."""
+    import torch
+    dev = torch.device("cuda:0")
+    a = inputs.random_state(70, 60, 50, seed=11, vamp=1.0)
+    b = inputs.random_state(70, 60, 50, seed=12, vamp=4.0)
+    Ud = torch.from_numpy(a).to(dev)
+    smax = torch.zeros(1, dtype=torch.float64, device=dev)
+    flag = torch.zeros(1, dtype=torch.int32, device=dev)
+    binding.max_signal_speed_noalloc(Ud, 1.4, smax, flag)
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        binding.max_signal_speed_noalloc(Ud, 1.4, smax, flag)       # on the capturing stream
+    for U in (a, b, a):
+        Ud.copy_(torch.from_numpy(U))
+        smax.fill_(-1.0)
+        flag.fill_(-1)
+        graph.replay()
+        torch.cuda.synchronize()
+        assert flag.item() == 0 and _same(smax.item(), _existing(U, 1.4, False), False)
+
+
 def test_sizes_beyond_the_scratch_are_rejected_without_a_device():
     """Argument errors come before any CUDA call: a size beyond HYDRO_NOALLOC_MAX_CELLS (the capacity of
     the static scratch array), an empty state, a NULL pointer, gamma <= 1."""
