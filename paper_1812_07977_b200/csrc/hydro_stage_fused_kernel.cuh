@@ -222,6 +222,14 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         const double *Uk = sm + S::OFF_RING + ((c + 2) % FNS) * S::STAGE;      // raw plane of cell plane c
         const long long cg = col + g.sy * (long long)(k0 + c + NG);
         double *Wsm = sm + S::OFF_W + (PIPE ? (c & 1) * S::STAGE : 0);
+        // stage 2 reads its own U0 values with plain loads behind the flux hand-off (no shared memory left to
+        // stage them through); their DRAM latency showed up as long-scoreboard stalls on the first use.  Lanes
+        // 0..4 of every warp ask L2 for the warp's row of the NEXT plane, one variable each: one instruction
+        // per warp and plane (256^3: stage 2 -2.0 %, 512^3: -4.5 %; two planes ahead: the same, three: less).
+        if (STAGE == 2 && tx < NVAR && j0 + ty < g.ny && c + 1 < nc) {
+            const int ncell = min(TX, g.nx - i0) & ~1;              // whole 16-byte units
+            if (ncell > 0) tma::prefetch_l2(a.Uold + tx * sv + (cg - tx) + g.sy, (uint32_t)ncell * 8u);
+        }
         if (!PIPE) tma::mbar_wait(barW, par);
         // ---- P2: x and y slopes of the own cell (W(k) = Wa), outer face values out ----------
         double Ix[5], Iy[5];

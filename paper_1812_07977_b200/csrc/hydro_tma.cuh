@@ -29,6 +29,13 @@ __device__ __forceinline__ void fence_barrier_init()
 }
 
 // generic-proxy accesses before, async-proxy (TMA) accesses after
+// L2 prefetch of `bytes` (multiple of 16) from the 16-byte aligned global address `p`: one instruction, no
+// destination, no completion to wait for (stage 2 warms the lines its plain U0 loads will read a plane later)
+__device__ __forceinline__ void prefetch_l2(const void *p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
