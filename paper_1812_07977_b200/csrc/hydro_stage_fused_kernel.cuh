@@ -224,11 +224,12 @@ stage_fused_kernel(const __grid_constant__ CUtensorMap umap, const FusedArgs a)
         double *Wsm = sm + S::OFF_W + (PIPE ? (c & 1) * S::STAGE : 0);
         // stage 2 reads its own U0 values with plain loads behind the flux hand-off (no shared memory left to
         // stage them through); their DRAM latency showed up as long-scoreboard stalls on the first use.  Lanes
-        // 0..4 of every warp ask L2 for the warp's row of the NEXT plane, one variable each: one instruction
-        // per warp and plane (256^3: stage 2 -2.0 %, 512^3: -4.5 %; two planes ahead: the same, three: less).
-        if (STAGE == 2 && tx < NVAR && j0 + ty < g.ny && c + 1 < nc) {
-            const int ncell = min(TX, g.nx - i0) & ~1;              // whole 16-byte units
-            if (ncell > 0) tma::prefetch_l2(a.Uold + tx * sv + (cg - tx) + g.sy, (uint32_t)ncell * 8u);
+        // 0..9 of every warp ask L2 for the warp's row of the NEXT plane, one 128-byte line each (variable
+        // lane / 2, half lane % 2): one instruction per warp and plane (256^3: stage 2 -3.4 %, 128^3: -3.9 %,
+        // 512^3: -4 %; two planes ahead: the same, three: less).
+        if (STAGE == 2 && tx < 2 * NVAR && j0 + ty < g.ny && c + 1 < nc) {
+            const int v = tx >> 1, half = tx & 1;
+            if (half * 16 < g.nx - i0) tma::prefetch_l2_line(a.Uold + v * sv + (cg - tx) + g.sy + half * 16);
         }
         if (!PIPE) tma::mbar_wait(barW, par);
         // ---- P2: x and y slopes of the own cell (W(k) = Wa), outer face values out ----------

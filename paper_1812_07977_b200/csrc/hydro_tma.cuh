@@ -29,11 +29,13 @@ __device__ __forceinline__ void fence_barrier_init()
 }
 
 // generic-proxy accesses before, async-proxy (TMA) accesses after
-// L2 prefetch of `bytes` (multiple of 16) from the 16-byte aligned global address `p`: one instruction, no
-// destination, no completion to wait for (stage 2 warms the lines its plain U0 loads will read a plane later)
-__device__ __forceinline__ void prefetch_l2(const void *p, uint32_t bytes)
+// L2 prefetch of the 128-byte line that holds `p`: one instruction for the lanes that call it, no destination,
+// nothing to wait for (stage 2 warms the lines its plain U0 loads will read a plane later).  The bulk form
+// (cp.async.bulk.prefetch.L2 = UBLKPF.L2) takes uniform-register operands: the compiler wraps it in a loop
+// over the active lanes, seven instructions per lane -- measured slower than this per-lane form.
+__device__ __forceinline__ void prefetch_l2_line(const void *p)
 {
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
 }
 
 __device__ __forceinline__ void fence_proxy_async()
