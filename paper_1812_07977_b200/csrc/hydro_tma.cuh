@@ -28,7 +28,6 @@ __device__ __forceinline__ void fence_barrier_init()
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 
-// generic-proxy accesses before, async-proxy (TMA) accesses after
 // L2 prefetch of the 128-byte line that holds `p`: one instruction for the lanes that call it, no destination,
 // nothing to wait for (stage 2 warms the lines its plain U0 loads will read a plane later).  The bulk form
 // (cp.async.bulk.prefetch.L2 = UBLKPF.L2) takes uniform-register operands: the compiler wraps it in a loop
@@ -38,6 +37,7 @@ __device__ __forceinline__ void prefetch_l2_line(const void *p)
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p) : "memory");
 }
 
+// generic-proxy accesses before, async-proxy (TMA) accesses after
 __device__ __forceinline__ void fence_proxy_async()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
